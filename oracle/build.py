@@ -1,0 +1,27 @@
+"""Build the fp64 CPU oracle (oracle/birkhoff4_oracle.c -> oracle/libbirkhoff4_oracle.so) with gcc.
+
+TEST INFRASTRUCTURE: the product (paper_2606_07574_b200) never imports or links this.
+Run as `python -m oracle.build`; `__graft_entry__.build()` and the test fixtures call `build()`.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "birkhoff4_oracle.c")
+LIB = os.path.join(HERE, "libbirkhoff4_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+        return LIB
+    # no -ffast-math: the oracle must keep IEEE semantics (NaN/Inf propagation, exact rounding order)
+    cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-Wall", "-Wextra",
+           "-o", LIB + ".tmp", SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(LIB + ".tmp", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))
