@@ -1,0 +1,124 @@
+/*
+ * birkhoff4.h -- C ABI of libbirkhoff4.so: batched 4x4 Birkhoff (KL / entropic-OT) projection on one B200.
+ *
+ * Source of every operation: arXiv 2606.07574 ("PAPER.md" = /root/reference/PAPER.md at build time).
+ *
+ *   forward   P = proj^KL_{B_4}(exp(H)) = diag(u) exp(H) diag(v), unit row and column sums
+ *             (eq. (1); Sinkhorn's theorem PAPER.md:62), found by Newton's method on the
+ *             gauge-fixed 3-variable dual f(beta_1..3) (eq. (8)) with the closed-form
+ *             gradient and 3x3 Hessian (eq. (9)-(11) PAPER.md:144-221), a guarded step
+ *             and a stop on marginal error.
+ *   backward  dL/dH from P and dL/dP by the implicit-function-theorem formula, no stored iterates
+ *             (eq. (13), 4x4 case PAPER.md:284-304; dL/dH = -D).
+ *   sinkhorn  K = exp(H), n_iter x (row-normalise, column-normalise): the Sinkhorn-20 baseline the
+ *             paper compares against (eq. (2)).
+ *
+ * Conventions (all entry points)
+ *   layout     [B][4][4] row-major contiguous: element (i,j) of matrix b at 16*b + 4*i + j.
+ *              H is the paper's R = -M.
+ *   pointers   DEVICE pointers unless the name ends in _host; owned by the caller.  The library never
+ *              allocates or frees device memory in the device-pointer calls and never synchronises:
+ *              every call is asynchronous on `stream` (a cudaStream_t; 0 = the legacy default stream).
+ *   alignment  every matrix pointer must be 32-byte aligned (else BIRKHOFF4_EINVAL; there is no slow path).
+ *   aliasing   P == H and dH == dP are allowed as exact aliases; partial overlap is undefined.
+ *   errors     return 0 on success; BIRKHOFF4_EINVAL for a null pointer with B > 0, B < 0, tol < 0 or NaN,
+ *              max_iter < 0, n_iter < 0 or a misaligned pointer; BIRKHOFF4_ECUDA_BASE + cudaError_t if
+ *              the launch failed.  B == 0 is a successful no-op.
+ *   NaN/Inf    a matrix holding a NaN or Inf gives an all-NaN output for that matrix only; the loops
+ *              are bounded by max_iter, so nothing hangs.
+ *   precision  fp32 storage and arithmetic (exp on the SFU via ex2.approx); bf16 inputs are widened
+ *              exactly to fp32.
+ *
+ * There is no CPU fallback: without a CUDA device every compute call returns an error.
+ */
+#ifndef BIRKHOFF4_H
+#define BIRKHOFF4_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BIRKHOFF4_OK 0
+#define BIRKHOFF4_EINVAL 1
+#define BIRKHOFF4_ECUDA_BASE 1000 /* return value = BIRKHOFF4_ECUDA_BASE + cudaError_t */
+
+#define BIRKHOFF4_HIST_BINS 64
+
+typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
+
+/*
+ * Forward projection (section 3).  H, P: device, fp32 [B][4][4].
+ *   tol       stop when the marginal error Err(T) = ||T1-1||_1 + ||T^T1-1||_1 of the
+ *             current iterate is <= tol.  Rows of T are normalised by construction (eq. (10)), so the
+ *             kernel tests the column part |g1|+|g2|+|g3|+|g1+g2+g3|, g = c - 1 (eq. (11)), in fp32
+ *             against an internal threshold min(tol, max(tol/2, tol - 5e-7)) that leaves room for the
+ *             fp32 rounding of the rows (S3/S9).  tol = 0 runs to the fp32 floor.
+ *   max_iter  maximum number of updates of beta per matrix (Newton steps plus fallback column
+ *             steps; PAPER.md:319 uses 20).  Function evaluations <= max_iter + 2 (one extra
+ *             for the start-up column step, S1).
+ * A matrix that has not converged after max_iter updates gets its last iterate (rows still
+ * normalised); this is not an error (Table 2 reports such iterates too).
+ */
+int birkhoff4_forward(const float* H, float* P, int64_t B, float tol, int max_iter, birkhoff4_stream_t stream);
+
+/*
+ * Forward with diagnostics.  Extra outputs, each nullable:
+ *   iters          int32 [B]: updates of beta taken by each matrix (0..max_iter)
+ *   hist           uint64 [BIRKHOFF4_HIST_BINS]: hist[k] += #matrices with min(iters, 63) == k
+ *                  (accumulated with atomics: zero it before the call)
+ *   n_unconverged  uint64 [1]: += #matrices that stopped on max_iter or at the fp32 floor with the
+ *                  tested error still above the internal threshold
+ */
+int birkhoff4_forward_ex(const float* H, float* P, int64_t B, float tol, int max_iter, int32_t* iters,
+                         unsigned long long* hist, unsigned long long* n_unconverged,
+                         birkhoff4_stream_t stream);
+
+/* Forward for logits stored as bf16 bit patterns (uint16 [B][4][4], 32 B per matrix); P is fp32. */
+int birkhoff4_forward_bf16(const uint16_t* H, float* P, int64_t B, float tol, int max_iter,
+                           birkhoff4_stream_t stream);
+
+/*
+ * Backward (section 4.2).  P: the forward output; dP = dL/dP; dH = dL/dH, all
+ * device fp32 [B][4][4].  Gamma = dP o P, mu_r = Gamma 1, mu_c = Gamma^T 1, w_{1..3} from the 3x3
+ * system Delta w = mu_c - P_{-4}^T mu_r (w_4 = 0), v = mu_r - P w, dH_ij = P_ij (dP_ij - v_i - w_j).
+ * Delta is formed and solved as a grounded graph Laplacian by node elimination (S7), which
+ * stays finite when P is (near) a permutation.
+ */
+int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, birkhoff4_stream_t stream);
+
+/*
+ * Sinkhorn-Knopp baseline (eq. (2)): K = exp(H) (row-max shifted, which the first row
+ * normalisation cancels), then n_iter x (rows /= row sums; columns /= column sums).  n_iter = 20 is the
+ * "Sinkhorn-20" of PAPER.md:32, 319.  Reported baseline only.
+ */
+int birkhoff4_sinkhorn(const float* H, float* P, int64_t B, int n_iter, birkhoff4_stream_t stream);
+
+/*
+ * Host-buffer convenience calls (end-to-end path): H_host/dP_host/P_host/dH_host are HOST pointers
+ * (pinned memory recommended; pageable works but copies then serialise).  The batch is cut into
+ * chunks that are copied to the device, processed and copied back on a small ring of internal
+ * streams and device buffers (allocated on first use, released by birkhoff4_host_release()).
+ * These calls are synchronous: they return when the outputs are in host memory.
+ *   birkhoff4_forward_host           H_host -> P_host
+ *   birkhoff4_backward_host          P_host, dP_host -> dH_host
+ *   birkhoff4_forward_backward_host  H_host, dP_host -> P_host (nullable), dH_host
+ *                                    (P stays on the device between the two kernels)
+ */
+int birkhoff4_forward_host(const float* H_host, float* P_host, int64_t B, float tol, int max_iter);
+int birkhoff4_backward_host(const float* P_host, const float* dP_host, float* dH_host, int64_t B);
+int birkhoff4_forward_backward_host(const float* H_host, const float* dP_host, float* P_host, float* dH_host,
+                                    int64_t B, float tol, int max_iter);
+void birkhoff4_host_release(void);
+
+/* Select the forward kernel variant (for measurement): 0 = library default.  Returns the previous value. */
+int birkhoff4_set_variant(int variant);
+
+const char* birkhoff4_strerror(int code);
+int birkhoff4_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIRKHOFF4_H */

@@ -5,4 +5,4 @@ package is a thin ctypes binding with the same entry-point names (`binding.py`),
 (`build.py`) and the seeded workload generators (`inputs.py`).  There is no CPU fallback: every
 compute call raises if the CUDA library is missing.
 """
-__all__ = ["inputs"]
+__all__ = ["inputs", "binding", "build"]

@@ -1,0 +1,404 @@
+// bk4_core.cuh -- per-matrix solvers of the batched 4x4 Birkhoff projection, written once for the value
+// types of bk4_vec.cuh (float: one matrix per thread; float2: two matrices per thread, packed FP32).
+//
+// Citations are to /root/reference/PAPER.md (arXiv 2606.07574); "DESIGN.md Sx/Gx" are the readings of the
+// passages where the paper is silent or garbled.
+//
+// Notation (paper): R = H (logits), U_ij = beta_j + R_ij, T = row-softmax(U) (eq. (10)), c = column sums,
+// g = c_{1..3} - 1 (eq. (11)), Hessian = diag(c) - T_{-4}^T T_{-4}.
+//
+// How T(beta) is evaluated here: write beta = beta0 + delta and
+// keep E_ij = exp(U0_ij - mu_i) for the base point beta0 (16 exponentials, once) and v_j = exp(delta_j).
+// Then T_ij = E_ij v_j / sum_k E_ik v_k is eq. (10) exactly, a Newton update beta += d is v_j *= exp(d_j)
+// (3 exponentials instead of 16), and the row-max shift mu_i keeps every exponential <= 1 as in PAPER.md:186-191.
+// When |delta| grows past 2^40 the base is moved (beta0 += delta, E recomputed from H).
+#pragma once
+#include "bk4_vec.cuh"
+
+#ifndef BK4_TRACE  // development hook (host emulation of the solver); compiles to nothing in the library
+#define BK4_TRACE(...)
+#endif
+
+namespace bk4 {
+
+constexpr float kLog2e = 1.4426950408889634f;
+#define kInf __int_as_float(0x7f800000)
+#define kNaN __int_as_float(0x7fc00000)
+constexpr float kVHi = 1.099511627776e12f;   // 2^40: range of v before the base point is moved
+constexpr float kVLo = 9.094947017729282e-13f;  // 2^-40
+// 2^-22 added to the three ground weights of the Laplacian (Hessian and Delta), S7: a group of columns
+// whose link to column 4 is weaker than this carries a residual below it, and without it the rounding noise of
+// g divided by a vanishing link would throw the whole group by 2^60.
+constexpr float kLamGround = 2.384185791015625e-07f;
+
+// -------------------------------------------------------------------------------------------------
+// Solve the grounded graph Laplacian system  L d = -g  (3 unknowns), L = [[a+b+p, -a, -b], [-a, a+c+q, -c],
+// [-b, -c, b+c+r]].  This is the Newton system H d = -g of eq. (12) PAPER.md:223-233 (and Delta w = rhs of
+// eq. (13)) with H = diag(c) - T_{-4}^T T_{-4} written through its six edge weights
+// W_jk = sum_i T_ij T_ik >= 0: a,b,c = W12,W13,W23 and ground weights p,q,r = W14,W24,W34 (rows of T sum to 1,
+// so h_jj = sum_{k != j} W_jk; no subtraction c_j - sum_i T_ij^2 is formed).  Node elimination: every pivot
+// is a sum of non-negative terms (S7); `lam` on the ground weights keeps them non-zero when T is a
+// permutation matrix.  3 reciprocals on the SFU.
+template <class V>
+BK4_DEV void solve_grounded_laplacian(V a, V b, V c, V p, V q, V r, V g1, V g2, V g3, float lam, V& d1, V& d2,
+                                      V& d3) {
+    const V l = vsplat(V{}, lam);
+    p = vadd(p, l);
+    q = vadd(q, l);
+    r = vadd(r, l);
+    // eliminate node 1
+    const V i1 = vrcp(vadd(vadd(a, b), p));
+    const V ai = vmul(a, i1), bi = vmul(b, i1);
+    const V c2 = vfma(ai, b, c);
+    const V q2 = vfma(ai, p, q);
+    const V r2 = vfma(bi, p, r);
+    const V g2p = vfma(ai, g1, g2);
+    const V g3p = vfma(bi, g1, g3);
+    // eliminate node 2
+    const V i2 = vrcp(vadd(c2, q2));
+    const V ci = vmul(c2, i2);
+    const V r3 = vfma(ci, q2, r2);
+    const V g3pp = vfma(ci, g2p, g3p);
+    // back substitution
+    d3 = vneg(vmul(g3pp, vrcp(r3)));
+    d2 = vmul(vsub(vmul(c2, d3), g2p), i2);
+    d1 = vmul(vsub(vfma(a, d2, vmul(b, d3)), g1), i1);
+}
+
+// six edge weights W_jk = sum_i T_ij T_ik of the column graph (the p_jk dot products)
+template <class V>
+BK4_DEV V col_dot(const V (&T)[16], int j, int k) {
+    return vfma(T[12 + j], T[12 + k], vfma(T[8 + j], T[8 + k], vfma(T[4 + j], T[4 + k], vmul(T[j], T[k]))));
+}
+
+// E_ij = 2^(u_ij - mu_i), u_ij = H_ij log2(e) + b0_j, mu_i = max_j u_ij  (eq. (10) PAPER.md:186-191 at the base
+// point beta0 = b0 / log2(e); b0_4 = 0 is the gauge PAPER.md:132).  First call (b0 = 0): `zero_base`.
+template <class V>
+BK4_DEV void base_exponentials(const V (&H)[16], const V (&b0)[3], bool zero_base, V (&E)[16]) {
+    const V l2e = vsplat(V{}, kLog2e);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (zero_base) {
+            const V m = vmax(vmax(H[4 * i], H[4 * i + 1]), vmax(H[4 * i + 2], H[4 * i + 3]));
+            const V t = vmul(m, vsplat(V{}, -kLog2e));
+#pragma unroll
+            for (int j = 0; j < 4; ++j) E[4 * i + j] = vex2(vfma(H[4 * i + j], l2e, t));
+        } else {
+            V u[4];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) u[j] = vfma(H[4 * i + j], l2e, b0[j]);
+            u[3] = vmul(H[4 * i + 3], l2e);
+            const V m = vmax(vmax(u[0], u[1]), vmax(u[2], u[3]));
+#pragma unroll
+            for (int j = 0; j < 4; ++j) E[4 * i + j] = vex2(vsub(u[j], m));
+        }
+    }
+}
+
+// T(beta) of eq. (10) from the base exponentials and v = exp(delta): rows normalised, plus the column residuals
+// g_j = c_j - 1 for all four columns.  Two details keep the fp32 floor of Err below 1e-6 (S9):
+// the SFU reciprocal (1 ulp) gets one Newton-Raphson refinement so that rows sum to 1 within rounding, and
+// the residual is summed as sum_i (T_ij - 1/4), whose partial sums are small, instead of (sum_i T_ij) - 1.
+template <class V>
+BK4_DEV void eval_T(const V (&E)[16], const V (&v)[3], V (&T)[16], V (&g)[4]) {
+    const V one = vsplat(V{}, 1.0f), mq = vsplat(V{}, -0.25f);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const V x0 = vmul(E[4 * i], v[0]), x1 = vmul(E[4 * i + 1], v[1]), x2 = vmul(E[4 * i + 2], v[2]);
+        const V x3 = E[4 * i + 3];
+        const V s = vadd(vadd(x0, x1), vadd(x2, x3));
+        const V r0 = vrcp(s);
+        const V r = vfma(r0, vfma(vneg(s), r0, one), r0);
+        T[4 * i] = vmul(x0, r);
+        T[4 * i + 1] = vmul(x1, r);
+        T[4 * i + 2] = vmul(x2, r);
+        T[4 * i + 3] = vmul(x3, r);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+        g[j] = vadd(vadd(vadd(T[j], mq), vadd(T[4 + j], mq)), vadd(vadd(T[8 + j], mq), vadd(T[12 + j], mq)));
+}
+
+template <class V>
+BK4_DEV V clamp_ratio(V x) {
+    // keeps a column step finite when a column sum underflows (NaN passes through vmin/vmax as the other operand,
+    // which is fine: a NaN matrix is caught by the error test)
+    return vmin(vmax(x, vsplat(V{}, kVLo)), vsplat(V{}, kVHi));
+}
+
+// -------------------------------------------------------------------------------------------------
+// Start point for large-magnitude logits (S1).  As |H| grows the projection tends to the
+// max-weight assignment (the LP limit eta -> 0 of (3)), and from beta = 0 both Newton and Sinkhorn
+// need O(range) steps.  This start takes the LP's dual potentials instead:
+//   1. sigma = argmax over the 24 permutations of sum_i H_{i,sigma(i)}  (brute force, shared pair sums);
+//   2. in the column order that puts sigma on the diagonal, x is dual-feasible iff x_j - x_k <= w_kj :=
+//      H_kk - H_kj for all k != j (then every assigned entry is its row's maximum of U = H + x);
+//      all-pairs shortest paths d of w (Floyd-Warshall, 4 nodes) give the feasible extremes x = d[s][.] and
+//      x = -d[.][t]; their average over all s, t is feasible too and sits inside the dual polytope, so that
+//      unassigned entries start e^{-slack} small instead of tied;
+//   3. beta0_j = x_{sigma^{-1}(j)} - x_{sigma^{-1}(4)}   (gauge beta_4 = 0), returned in log2 units.
+// Indices are carried as float values 0..3 so that the code is the same for both value types; everything is
+// selects and static indexing (no local memory).
+template <class V>
+BK4_DEV void lp_dual_start(const V (&H)[16], V (&b0)[3]) {
+    using M = typename vtraits<V>::mask;
+    const V c0 = vsplat(V{}, 0.0f), c1 = vsplat(V{}, 1.0f), c2 = vsplat(V{}, 2.0f), c3 = vsplat(V{}, 3.0f);
+    const V cidx[4] = {c0, c1, c2, c3};
+    // 1. best permutation.  Rows 0,1 take the ordered pair (j0,j1); rows 2,3 take the other two columns in the
+    //    better of their two orders.
+    V best = vsplat(V{}, -kInf), s0 = c0, s1 = c1, s2 = c2, s3 = c3;
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = a + 1; b < 4; ++b) {
+            // complement pair {a,b} for rows 2,3
+            const V bab = vadd(H[8 + a], H[12 + b]), bba = vadd(H[8 + b], H[12 + a]);
+            const M f = vgt(bba, bab);
+            const V bb = vmax(bab, bba);
+            const V t2 = vsel(f, cidx[b], cidx[a]), t3 = vsel(f, cidx[a], cidx[b]);
+            int p = 0, q = 0;  // the two columns left for rows 0,1
+            for (int j = 0, n = 0; j < 4; ++j)
+                if (j != a && j != b) {
+                    if (n++ == 0) p = j;
+                    else q = j;
+                }
+#pragma unroll
+            for (int o = 0; o < 2; ++o) {
+                const int j0 = o ? q : p, j1 = o ? p : q;
+                const V S = vadd(vadd(H[j0], H[4 + j1]), bb);
+                const M m = vgt(S, best);
+                best = vsel(m, S, best);
+                s0 = vsel(m, cidx[j0], s0);
+                s1 = vsel(m, cidx[j1], s1);
+                s2 = vsel(m, t2, s2);
+                s3 = vsel(m, t3, s3);
+            }
+        }
+    // 2. columns reordered so that the assignment is the diagonal: Hc[i][m] = H[i][sigma(m)]
+    const V sg[4] = {s0, s1, s2, s3};
+    M eq[4][3];
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) eq[m][j] = veq(sg[m], cidx[j]);
+    V Hc[16];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int m = 0; m < 4; ++m)
+            Hc[4 * i + m] = vsel(eq[m][0], H[4 * i], vsel(eq[m][1], H[4 * i + 1], vsel(eq[m][2], H[4 * i + 2], H[4 * i + 3])));
+    V d[4][4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) d[k][j] = (k == j) ? c0 : vsub(Hc[5 * k], Hc[4 * k + j]);
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (k != m && j != m && k != j) d[k][j] = vmin(d[k][j], vadd(d[k][m], d[m][j]));
+    V x[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        V acc = c0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (k != j) acc = vadd(acc, vsub(d[k][j], d[j][k]));
+        x[j] = acc;  // 8 x the centre
+    }
+    // 3. back to the original column order, gauge, log2 units
+    V beta[4];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) beta[j] = vsel(eq[0][j], x[0], vsel(eq[1][j], x[1], vsel(eq[2][j], x[2], x[3])));
+    {
+        const M e0 = mor(mor(eq[0][0], eq[0][1]), eq[0][2]), e1 = mor(mor(eq[1][0], eq[1][1]), eq[1][2]),
+                e2 = mor(mor(eq[2][0], eq[2][1]), eq[2][2]);
+        beta[3] = vsel(e0, vsel(e1, vsel(e2, x[3], x[2]), x[1]), x[0]);
+    }
+    const V sc = vsplat(V{}, 0.125f * kLog2e);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) b0[j] = vmul(vsub(beta[j], beta[3]), sc);
+}
+
+// -------------------------------------------------------------------------------------------------
+// Guarded Newton on f(beta_1..3) (eq. (8); iteration PAPER.md:164-168).
+//
+//   start     beta0 = 0, or the LP dual start above for the matrices flagged `hard` (large logit range),
+//             followed by one Sinkhorn-Knopp column step (eq. (6)) -- DESIGN.md S1
+//   step      d = -Hessian^{-1} g  (eq. (9),(11),(12))
+//   guard     accept the full step iff the column residual err decreased; otherwise go back and take a
+//             Sinkhorn column step beta_j -= log(c_j / c_4), which never increases err -- DESIGN.md S2
+//   stop      err = |g1|+|g2|+|g3|+|g1+g2+g3| <= tol_i (rows are exact by eq. (10)) -- S3;
+//             after max_iter updates -- S4; or when neither step lowers err (fp32 floor) -- S5
+//
+// `any_hard` must be uniform over the threads that execute together (it only selects the cheaper start-up
+// code when no matrix needs the LP start).  Reload(H) re-reads the logits (used when the base point moves);
+// Emit(half, T, iters, converged) receives the result of one matrix as soon as it is final.
+template <class V, class Reload, class Emit>
+BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bool any_hard, float tol_i,
+                            int max_iter, Reload&& reload, Emit&& emit) {
+    using M = typename vtraits<V>::mask;
+    constexpr int NL = vtraits<V>::lanes;
+    const V one = vsplat(V{}, 1.0f), zero = vsplat(V{}, 0.0f);
+
+    V E[16], T[16], c[4], v[3], b0[3];
+    b0[0] = b0[1] = b0[2] = zero;
+    if (any_hard) {
+        V bl[3];
+        lp_dual_start(H, bl);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) b0[j] = vsel(hard, bl[j], zero);
+        base_exponentials(H, b0, false, E);
+    } else {
+        base_exponentials(H, b0, true, E);
+    }
+
+    // start-up column step (v = 1): v_j = c_4 / c_j
+    v[0] = v[1] = v[2] = one;
+    eval_T(E, v, T, c);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) v[j] = clamp_ratio(vmul(vadd(c[3], one), vrcp(vadd(c[j], one))));
+
+    V vprev[3] = {v[0], v[1], v[2]}, cprev[4] = {zero, zero, zero, zero};
+    V errprev = vsplat(V{}, kInf);
+    M newton_trial = msplat(V{}, false), sink_trial = msplat(V{}, false), done = msplat(V{}, false);
+    int it[NL];
+#pragma unroll
+    for (int k = 0; k < NL; ++k) it[k] = 0;
+    const V tolv = vsplat(V{}, tol_i);
+
+    for (;;) {
+        eval_T(E, v, T, c);  // c holds the residuals c_j - 1
+        const V g1 = c[0], g2 = c[1], g3 = c[2];
+        const V err = vadd(vadd(vabs(g1), vabs(g2)), vadd(vabs(g3), vabs(c[3])));
+        const M conv = mnot(vgt(err, tolv));  // NaN counts as "stop"
+        const M improved = vlt(err, errprev);
+        const M rej = mand(mand(newton_trial, mnot(improved)), mnot(conv));
+        const M stag = mand(mand(sink_trial, mnot(improved)), mnot(conv));
+        M capped;
+        if constexpr (NL == 1) capped = it[0] >= max_iter;
+        else capped = M{it[0] >= max_iter, it[1] >= max_iter};
+        const M fin = mor(mor(conv, capped), stag);
+        BK4_TRACE("it %d err %.3e errprev %.3e v %.3e %.3e %.3e c %.4f %.4f %.4f %.4f rej %d stag %d\n", it[0],
+                  vget(err, 0), vget(errprev, 0), vget(v[0], 0), vget(v[1], 0), vget(v[2], 0), 1 + vget(c[0], 0),
+                  1 + vget(c[1], 0), 1 + vget(c[2], 0), 1 + vget(c[3], 0), (int)mget(rej, 0), (int)mget(stag, 0));
+#pragma unroll
+        for (int k = 0; k < NL; ++k)
+            if (mget(fin, k) && !mget(done, k)) emit(k, T, it[k], mget(conv, k));
+        done = mor(done, fin);
+        if (mall(done)) break;
+
+        const M act = mnot(done);
+        const M rejected = mand(rej, act);
+        const M accepted = mand(mnot(rej), act);
+
+        // accepted point far from the base: move the base there (beta0 += delta, E recomputed from H, v = 1).
+        // T, c and the Newton direction below do not depend on where the base is.
+        {
+            const V vmx = vmax(vmax(v[0], v[1]), v[2]), vmn = vmin(vmin(v[0], v[1]), v[2]);
+            const M far = mand(accepted, mor(vgt(vmx, vsplat(V{}, kVHi)), vlt(vmn, vsplat(V{}, kVLo))));
+            if (many(far)) {
+                V Hr[16];
+                reload(Hr);
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    b0[j] = vsel(far, vadd(b0[j], vlg2(v[j])), b0[j]);
+                    v[j] = vsel(far, one, v[j]);
+                }
+                base_exponentials(Hr, b0, false, E);
+            }
+        }
+
+        V vn[3] = {v[0], v[1], v[2]};
+        if (many(accepted)) {
+            // Newton direction at the accepted point (eq. (12) through the Laplacian form, S7)
+            V d1, d2, d3;
+            solve_grounded_laplacian(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), col_dot(T, 0, 3),
+                                     col_dot(T, 1, 3), col_dot(T, 2, 3), g1, g2, g3, kLamGround, d1, d2, d3);
+            // beta += d  <=>  v *= exp(d).  The step is clipped to |d| <= 60 ln 2: a (near-)singular Hessian far
+            // from the solution gives an unbounded direction; the guard then decides.  With |log2 v| <= 40 at
+            // accepted points the trial stays inside the fp32 range.
+            const V l2e = vsplat(V{}, kLog2e), hi = vsplat(V{}, 60.0f), lo = vsplat(V{}, -60.0f);
+            vn[0] = vmul(v[0], vex2(vmin(vmax(vmul(d1, l2e), lo), hi)));
+            vn[1] = vmul(v[1], vex2(vmin(vmax(vmul(d2, l2e), lo), hi)));
+            vn[2] = vmul(v[2], vex2(vmin(vmax(vmul(d3, l2e), lo), hi)));
+        }
+        if (many(rejected)) {
+            // back to the last accepted point, Sinkhorn column step from there
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                const V vs = vmul(vprev[j], clamp_ratio(vmul(vadd(cprev[3], one), vrcp(vadd(cprev[j], one)))));
+                vn[j] = vsel(rejected, vs, vn[j]);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            vprev[j] = vsel(accepted, v[j], vprev[j]);
+            v[j] = vsel(act, vn[j], v[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) cprev[j] = vsel(accepted, c[j], cprev[j]);
+        errprev = vsel(accepted, err, errprev);
+        newton_trial = accepted;
+        sink_trial = rejected;
+#pragma unroll
+        for (int k = 0; k < NL; ++k) it[k] += mget(act, k) ? 1 : 0;
+    }
+}
+
+// -------------------------------------------------------------------------------------------------
+// Backward, PAPER.md:284-304 (section 4.2) with Delta solved as a grounded Laplacian (S6/S7):
+//   Gamma = G o P, mu_r = Gamma 1, mu_c = (Gamma^T 1)_{1..3}, rhs = mu_c - P_{-4}^T mu_r,
+//   Delta w = rhs, w_4 = 0, v = mu_r - P w, dH_ij = P_ij (G_ij - v_i - w_j)   ( = -D_ij, PAPER.md:302-304 )
+template <class V>
+BK4_DEV void backward_ift(const V (&P)[16], const V (&G)[16], V (&dH)[16]) {
+    V mur[4], muc[3], rhs[3];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+        mur[i] = vfma(G[4 * i + 3], P[4 * i + 3],
+                      vfma(G[4 * i + 2], P[4 * i + 2], vfma(G[4 * i + 1], P[4 * i + 1], vmul(G[4 * i], P[4 * i]))));
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        muc[j] = vfma(G[12 + j], P[12 + j], vfma(G[8 + j], P[8 + j], vfma(G[4 + j], P[4 + j], vmul(G[j], P[j]))));
+        const V pm = vfma(P[12 + j], mur[3], vfma(P[8 + j], mur[2], vfma(P[4 + j], mur[1], vmul(P[j], mur[0]))));
+        rhs[j] = vsub(muc[j], pm);
+    }
+    V w1, w2, w3;  // solve_grounded_laplacian returns -L^{-1} g: pass g = -rhs
+    solve_grounded_laplacian(col_dot(P, 0, 1), col_dot(P, 0, 2), col_dot(P, 1, 2), col_dot(P, 0, 3), col_dot(P, 1, 3),
+                             col_dot(P, 2, 3), vneg(rhs[0]), vneg(rhs[1]), vneg(rhs[2]), kLamGround, w1, w2, w3);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const V vi = vsub(mur[i], vfma(P[4 * i + 2], w3, vfma(P[4 * i + 1], w2, vmul(P[4 * i], w1))));
+        dH[4 * i] = vmul(P[4 * i], vsub(vsub(G[4 * i], vi), w1));
+        dH[4 * i + 1] = vmul(P[4 * i + 1], vsub(vsub(G[4 * i + 1], vi), w2));
+        dH[4 * i + 2] = vmul(P[4 * i + 2], vsub(vsub(G[4 * i + 2], vi), w3));
+        dH[4 * i + 3] = vmul(P[4 * i + 3], vsub(G[4 * i + 3], vi));
+    }
+}
+
+// -------------------------------------------------------------------------------------------------
+// Sinkhorn-Knopp baseline, eq. (2): K = exp(H), n_iter x (row normalise, column normalise).
+// The row-max shift is cancelled by the first row normalisation (it only avoids fp32 overflow).
+template <class V>
+BK4_DEV void sinkhorn_knopp(const V (&H)[16], int n_iter, V (&T)[16]) {
+    V b0[3] = {vsplat(V{}, 0.0f), vsplat(V{}, 0.0f), vsplat(V{}, 0.0f)};
+    base_exponentials(H, b0, true, T);
+    for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const V r = vrcp(vadd(vadd(T[4 * i], T[4 * i + 1]), vadd(T[4 * i + 2], T[4 * i + 3])));
+#pragma unroll
+            for (int j = 0; j < 4; ++j) T[4 * i + j] = vmul(T[4 * i + j], r);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const V r = vrcp(vadd(vadd(T[j], T[4 + j]), vadd(T[8 + j], T[12 + j])));
+#pragma unroll
+            for (int i = 0; i < 4; ++i) T[4 * i + j] = vmul(T[4 * i + j], r);
+        }
+    }
+}
+
+}  // namespace bk4
