@@ -115,13 +115,14 @@ __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H
             valid[k] = b0 + k < B;
             idx[k] = valid[k] ? b0 + k : b0;  // an odd tail duplicates the last matrix in the idle half
             load_logits<BF16>(H, idx[k], h[k]);
-            float hmax = h[k][0], hmin = h[k][0];
+            float hmax = h[k][0], hmin = h[k][0], poison = 0.0f;
 #pragma unroll
-            for (int q = 1; q < 16; ++q) {
+            for (int q = 0; q < 16; ++q) {
                 hmax = fmaxf(hmax, h[k][q]);
                 hmin = fminf(hmin, h[k][q]);
+                poison = __fmaf_rn(h[k][q], 0.0f, poison);  // NaN iff some logit is NaN or +-Inf (fmaxf skips NaN)
             }
-            bad[k] = !(hmax - hmin < kInf);  // +-Inf logit; a NaN logit poisons T through the arithmetic
+            bad[k] = !(poison == 0.0f);
             hard[k] = hmax - hmin > kHardRange;
         }
         // the LP dual start is compiled into a branch that a warp takes only if one of its matrices needs it
@@ -129,8 +130,8 @@ __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H
         if constexpr (NL == 2) any_hard = any_hard || hard[1];
         any_hard = __any_sync(__activemask(), any_hard);
         typename vtraits<V>::mask hardm;
-        if constexpr (NL == 1) hardm = hard[0];
-        else hardm = bool2{hard[0], hard[1]};
+        if constexpr (NL == 1) hardm = bool1(hard[0]);
+        else hardm = bool2(hard[0], hard[1]);
         V Hv[16];
 #pragma unroll
         for (int q = 0; q < 16; ++q) {

@@ -126,6 +126,18 @@ BK4_DEV V clamp_ratio(V x) {
     return vmin(vmax(x, vsplat(V{}, kVLo)), vsplat(V{}, kVHi));
 }
 
+// Sinkhorn-Knopp column step (eq. (6) PAPER.md:108 with the gauge beta_4 = 0): ratio_j = c_4 / c_j, from the
+// column sums themselves.  The residuals g_j = c_j - 1 of eval_T cannot be used here: a column that a bad
+// Newton step has emptied (c_j ~ 1e-9) would come back from g_j + 1 as 0 or 6e-8 and the step would overshoot.
+template <class V>
+BK4_DEV void column_ratios(const V (&T)[16], V (&ratio)[3]) {
+    V cs[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) cs[j] = vadd(vadd(T[j], T[4 + j]), vadd(T[8 + j], T[12 + j]));
+#pragma unroll
+    for (int j = 0; j < 3; ++j) ratio[j] = clamp_ratio(vmul(cs[3], vrcp(cs[j])));
+}
+
 // -------------------------------------------------------------------------------------------------
 // Start point for large-magnitude logits (S1).  As |H| grows the projection tends to the
 // max-weight assignment (the LP limit eta -> 0 of (3)), and from beta = 0 both Newton and Sinkhorn
@@ -258,10 +270,9 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
     // start-up column step (v = 1): v_j = c_4 / c_j
     v[0] = v[1] = v[2] = one;
     eval_T(E, v, T, c);
-#pragma unroll
-    for (int j = 0; j < 3; ++j) v[j] = clamp_ratio(vmul(vadd(c[3], one), vrcp(vadd(c[j], one))));
+    column_ratios(T, v);
 
-    V vprev[3] = {v[0], v[1], v[2]}, cprev[4] = {zero, zero, zero, zero};
+    V vprev[3] = {v[0], v[1], v[2]};
     V errprev = vsplat(V{}, kInf);
     M newton_trial = msplat(V{}, false), sink_trial = msplat(V{}, false), done = msplat(V{}, false);
     int it[NL];
@@ -278,8 +289,8 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
         const M rej = mand(mand(newton_trial, mnot(improved)), mnot(conv));
         const M stag = mand(mand(sink_trial, mnot(improved)), mnot(conv));
         M capped;
-        if constexpr (NL == 1) capped = it[0] >= max_iter;
-        else capped = M{it[0] >= max_iter, it[1] >= max_iter};
+        if constexpr (NL == 1) capped = M(it[0] >= max_iter);
+        else capped = M(it[0] >= max_iter, it[1] >= max_iter);
         const M fin = mor(mor(conv, capped), stag);
         BK4_TRACE("it %d err %.3e errprev %.3e v %.3e %.3e %.3e c %.4f %.4f %.4f %.4f rej %d stag %d\n", it[0],
                   vget(err, 0), vget(errprev, 0), vget(v[0], 0), vget(v[1], 0), vget(v[2], 0), 1 + vget(c[0], 0),
@@ -326,20 +337,19 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
             vn[2] = vmul(v[2], vex2(vmin(vmax(vmul(d3, l2e), lo), hi)));
         }
         if (many(rejected)) {
-            // back to the last accepted point, Sinkhorn column step from there
+            // back to the last accepted point (T is re-evaluated there: rare path, and T is dead until the next
+            // eval_T), Sinkhorn column step from it
+            V ratio[3], gdead[4];
+            eval_T(E, vprev, T, gdead);
+            column_ratios(T, ratio);
 #pragma unroll
-            for (int j = 0; j < 3; ++j) {
-                const V vs = vmul(vprev[j], clamp_ratio(vmul(vadd(cprev[3], one), vrcp(vadd(cprev[j], one)))));
-                vn[j] = vsel(rejected, vs, vn[j]);
-            }
+            for (int j = 0; j < 3; ++j) vn[j] = vsel(rejected, vmul(vprev[j], ratio[j]), vn[j]);
         }
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
             vprev[j] = vsel(accepted, v[j], vprev[j]);
             v[j] = vsel(act, vn[j], v[j]);
         }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) cprev[j] = vsel(accepted, c[j], cprev[j]);
         errprev = vsel(accepted, err, errprev);
         newton_trial = accepted;
         sink_trial = rejected;

@@ -1,0 +1,462 @@
+"""GPU parity: libbirkhoff4.so (through the ctypes binding, i.e. through the C ABI) against the fp64 oracle.
+
+Same seeded inputs on both sides (paper_2606_07574_b200.inputs); the oracle never sees a CUDA result.
+Gates (BASELINE.json north_star; readings S9/S10 in DESIGN.md):
+    max |P - P_oracle|                        <= 1e-5
+    max Err(P)  (fp64 on the stored fp32 P)   <= 1e-6   at N(0,1); reported per scale otherwise
+    dH: (i)  max|dH - dH_o| / max|dH_o|       <= 1e-4
+        (ii) max_b ||dH_b - dH_o,b||_inf / ||G_b||_inf      <= 1e-4
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+from paper_2606_07574_b200 import binding as bk, inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_P = 1e-5
+TOL_ERR = 1e-6
+TOL_DH = 1e-4
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def host(t):
+    torch.cuda.synchronize()
+    return t.cpu().numpy()
+
+
+def gpu_forward(H, **kw):
+    return host(bk.birkhoff4_forward(dev(H), **kw)).astype(np.float64)
+
+
+def dh_errors(dH, dH_o, G):
+    e1 = np.abs(dH - dH_o).max() / max(np.abs(dH_o).max(), 1e-300)
+    e2 = (np.abs(dH - dH_o).reshape(len(G), -1).max(1) / np.abs(G).reshape(len(G), -1).max(1)).max()
+    return e1, e2
+
+
+def check_forward_backward(oracle, H32, G32, H_for_oracle=None, P_gpu=None, err_gate=TOL_ERR, max_iter=20):
+    """full element-by-element parity of forward and backward on one batch; returns the measured errors"""
+    Ho = (H32 if H_for_oracle is None else H_for_oracle).astype(np.float64)
+    P_o, info = oracle.forward(Ho, return_info=True)
+    ok = info["err"] <= oracle.CERTIFY
+    assert ok.mean() > 0.999, "oracle uncertified on too many matrices"
+    if P_gpu is None:
+        P_gpu = bk.birkhoff4_forward(dev(H32), max_iter=max_iter)
+    P = host(P_gpu).astype(np.float64)
+    assert np.isfinite(P).all()
+    eP = np.abs(P - P_o)[ok].max()
+    err = oracle.marginal_err(P)
+    assert eP <= TOL_P, "max|P-P_o| = %.3e" % eP
+    assert err.max() <= err_gate, "max Err = %.3e" % err.max()
+    dH = host(bk.birkhoff4_backward(P_gpu, dev(G32))).astype(np.float64)
+    dH_o = oracle.backward(P_o, G32.astype(np.float64))
+    assert np.isfinite(dH).all()
+    e1, e2 = dh_errors(dH[ok], dH_o[ok], G32[ok])
+    assert e1 <= TOL_DH and e2 <= TOL_DH, "dH errors %.3e %.3e" % (e1, e2)
+    return dict(eP=eP, err=err.max(), err_inf=oracle.marginal_err_inf(P).max(), e1=e1, e2=e2)
+
+
+# ---------------------------------------------------------------------------------------------------
+# config 1 (BASELINE.json configs[0]): B = 1024, N(0,1), every element against the oracle
+@pytest.mark.parametrize("variant", [1, 2])
+def test_config1_full_parity(oracle, variant):
+    c = inputs.make(1)
+    old = bk.birkhoff4_set_variant(variant)
+    try:
+        r = check_forward_backward(oracle, c["H"], c["G"])
+    finally:
+        bk.birkhoff4_set_variant(old)
+    print("config1 variant", variant, r)
+
+
+# several tiles and a ragged tail, both thread mappings
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("B", [1, 2, 3, 31, 33, 255, 257, 1000, 4097, 70001])
+def test_ragged_sizes(oracle, variant, B):
+    H, G = inputs.normal(B, 1.0, config=60, sub=B)
+    old = bk.birkhoff4_set_variant(variant)
+    try:
+        # guard cells around the output: nothing may be written past B matrices
+        buf = torch.full((B + 2, 4, 4), 7.0, device="cuda")
+        bk.birkhoff4_forward(dev(H), buf[1:B + 1])
+        assert (host(buf[0]) == 7.0).all() and (host(buf[B + 1]) == 7.0).all()
+        check_forward_backward(oracle, H, G, P_gpu=buf[1:B + 1].contiguous())
+        dbuf = torch.full((B + 2, 4, 4), 7.0, device="cuda")
+        bk.birkhoff4_backward(buf[1:B + 1], dev(G), dbuf[1:B + 1])
+        assert (host(dbuf[0]) == 7.0).all() and (host(dbuf[B + 1]) == 7.0).all()
+    finally:
+        bk.birkhoff4_set_variant(old)
+
+
+def test_empty_batch():
+    e = torch.empty((0, 4, 4), device="cuda")
+    assert bk.birkhoff4_forward(e).shape == (0, 4, 4)
+    assert bk.birkhoff4_backward(e, e).shape == (0, 4, 4)
+    assert bk.birkhoff4_sinkhorn(e).shape == (0, 4, 4)
+    L = bk.lib()
+    assert L.birkhoff4_forward(None, None, 0, 1e-6, 20, None) == 0       # B == 0: no-op even with null pointers
+
+
+# the paper's distributions (Tables 1-2) and the larger scales of config 3
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("s", [0.1, 1.0, 2.0, 3.0, 5.0, 10.0, 30.0, 100.0])
+def test_scales_parity(oracle, s, variant):
+    H, G = inputs.normal(8192, s, config=61)
+    old = bk.birkhoff4_set_variant(variant)
+    try:
+        r = check_forward_backward(oracle, H, G, err_gate=TOL_ERR if s <= 1.0 else 3e-6, max_iter=32)
+    finally:
+        bk.birkhoff4_set_variant(old)
+    print("scale", s, "variant", variant, r)
+
+
+@pytest.mark.parametrize("w", [1.0, 10.0])
+def test_uniform_parity(oracle, w):
+    H, G = inputs.uniform(8192, w, config=62)
+    r = check_forward_backward(oracle, H, G, err_gate=TOL_ERR if w <= 1.0 else 3e-6, max_iter=32)
+    print("uniform", w, r)
+
+
+# config 4: bf16 logits, fp32 P; the oracle gets the exactly widened values
+def test_config4_bf16_small(oracle):
+    c = inputs.make(4, B=8192 + 5)
+    Hb = torch.from_numpy(c["H"].view(np.int16)).cuda().view(torch.bfloat16)
+    P = bk.birkhoff4_forward_bf16(Hb)
+    r = check_forward_backward(oracle, c["H_f32"], c["G"], P_gpu=P, err_gate=3e-6)
+    # the bf16 entry point equals the fp32 entry point on the widened values, bit for bit
+    P32 = bk.birkhoff4_forward(dev(c["H_f32"]))
+    assert torch.equal(P, P32)
+    print("config4", r)
+
+
+# config 5: heterogeneous structure (near-permutations, duplicate rows, ties, scales 0.1..100)
+@pytest.mark.parametrize("variant", [1, 2])
+def test_config5_small(oracle, variant):
+    c = inputs.make(5, B=16384 + 7)
+    old = bk.birkhoff4_set_variant(variant)
+    try:
+        r = check_forward_backward(oracle, c["H"], c["G"], err_gate=3e-6, max_iter=32)
+    finally:
+        bk.birkhoff4_set_variant(old)
+    print("config5 variant", variant, r)
+
+
+# ---------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times: properties over the whole
+# output, the oracle on a sample of matrices
+def _full_size(oracle, H32, G32, P_gpu, n_sample, err_gate, seed):
+    B = H32.shape[0]
+    P = host(P_gpu)
+    assert np.isfinite(P).all()
+    P64 = P.astype(np.float64)
+    rows = np.abs(P64.sum(2) - 1).sum(1)
+    cols = np.abs(P64.sum(1) - 1).sum(1)
+    err = rows + cols                                                  # PAPER.md:323, all B matrices
+    assert err.max() <= err_gate, "max Err over %d matrices = %.3e" % (B, err.max())
+    assert P.min() >= 0.0
+    dH_gpu = bk.birkhoff4_backward(P_gpu, dev(G32))
+    dH = host(dH_gpu).astype(np.float64)
+    assert np.isfinite(dH).all()
+    scale = np.abs(G32).reshape(B, -1).max(1).astype(np.float64)
+    # P11: row and column sums of dH vanish (every matrix)
+    assert (np.abs(dH.sum(1)).max(1) / scale).max() < 2e-5
+    assert (np.abs(dH.sum(2)).max(1) / scale).max() < 2e-5
+    idx = np.sort(np.random.default_rng(seed).choice(B, n_sample, replace=False))
+    idx[0], idx[-1] = 0, B - 1
+    P_o, info = oracle.forward(H32[idx].astype(np.float64), return_info=True)
+    ok = info["err"] <= oracle.CERTIFY
+    eP = np.abs(P64[idx] - P_o)[ok].max()
+    assert eP <= TOL_P, "max|P-P_o| = %.3e" % eP
+    dH_o = oracle.backward(P_o, G32[idx].astype(np.float64))
+    e1, e2 = dh_errors(dH[idx][ok], dH_o[ok], G32[idx][ok])
+    assert e1 <= TOL_DH and e2 <= TOL_DH
+    return dict(eP=eP, err=err.max(), err_mean=err.mean(), e1=e1, e2=e2)
+
+
+def test_config2_full_size(oracle):
+    c = inputs.make(2)
+    P = bk.birkhoff4_forward(dev(c["H"]))
+    print("config2", _full_size(oracle, c["H"], c["G"], P, 8192, TOL_ERR, 2))
+
+
+@pytest.mark.parametrize("s", [10.0, 30.0, 100.0])
+def test_config3_full_size(oracle, s):
+    c = inputs.make(3, s=s)
+    hist = torch.zeros(64, dtype=torch.int64, device="cuda")
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    P = bk.birkhoff4_forward_ex(dev(c["H"]), max_iter=32, hist=hist, n_unconverged=unc)
+    r = _full_size(oracle, c["H"], c["G"], P, 2048, 3e-6, 3)
+    h = host(hist)
+    assert h.sum() == c["B"]
+    print("config3 s=%g" % s, r, "mean iters %.2f" % ((h * np.arange(64)).sum() / h.sum()), "max", np.nonzero(h)[0].max(),
+          "unconverged", int(host(unc)[0]))
+
+
+def test_config4_full_size(oracle):
+    c = inputs.make(4)
+    Hb = torch.from_numpy(c["H"].view(np.int16)).cuda().view(torch.bfloat16)
+    P = bk.birkhoff4_forward_bf16(Hb)
+    del Hb
+    print("config4", _full_size(oracle, c["H_f32"], c["G"], P, 4096, 3e-6, 4))
+
+
+def test_config5_full_size(oracle):
+    c = inputs.make(5)
+    P = bk.birkhoff4_forward(dev(c["H"]), max_iter=32)
+    print("config5", _full_size(oracle, c["H"], c["G"], P, 8192, 3e-6, 5))
+
+
+# ---------------------------------------------------------------------------------------------------
+# properties of the CUDA forward that hold at any size
+def test_separable_gives_uniform_gpu():
+    rng = np.random.default_rng(1)
+    a = rng.normal(size=(64, 4, 1)) * 5
+    b = rng.normal(size=(64, 1, 4)) * 5
+    H = np.concatenate([a + b, np.full((1, 4, 4), 3.25), np.zeros((1, 4, 4)), np.full((1, 4, 4), -1e4)]).astype(np.float32)
+    P = gpu_forward(H)
+    # fp32 H = a+b is separable only up to its own rounding (ulp(20) ~ 2e-6)
+    assert np.abs(P[:64] - 0.25).max() < 5e-6
+    assert np.abs(P[64:] - 0.25).max() < 1e-7
+
+
+def test_permutation_equivariance_gpu():
+    perms = list(itertools.permutations(range(4)))
+    for s in (1.0, 10.0):
+        H = inputs.normal(4, s, config=63)[0]
+        Hp = np.array([H[b][np.ix_(pr, pc)] for b in range(4) for pr in perms for pc in perms])
+        P = gpu_forward(H, max_iter=32)
+        want = np.array([P[b][np.ix_(pr, pc)] for b in range(4) for pr in perms for pc in perms])
+        assert np.abs(gpu_forward(Hp, max_iter=32) - want).max() < 2e-6
+
+
+def test_assignment_limit_gpu():
+    H = inputs.normal(1 << 16, 100.0, config=64)[0]
+    perms = np.array(list(itertools.permutations(range(4))))
+    tot = np.stack([sum(H[:, i, p[i]].astype(np.float64) for i in range(4)) for p in perms], axis=1)
+    order = np.sort(tot, axis=1)
+    keep = order[:, -1] - order[:, -2] > 160.0
+    best = perms[np.argmax(tot, axis=1)]
+    want = np.zeros((len(H), 4, 4))
+    for i in range(4):
+        want[np.arange(len(H)), i, best[:, i]] = 1.0
+    P = gpu_forward(H, max_iter=32)
+    assert keep.sum() > 1000
+    assert np.abs(P[keep] - want[keep]).max() < 1e-6
+
+
+def test_two_variants_agree_and_deterministic():
+    H = dev(inputs.normal(1 << 16, 3.0, config=65)[0])
+    bk.birkhoff4_set_variant(1)
+    a1, a2 = bk.birkhoff4_forward(H), bk.birkhoff4_forward(H)
+    bk.birkhoff4_set_variant(2)
+    b1 = bk.birkhoff4_forward(H)
+    bk.birkhoff4_set_variant(0)
+    assert torch.equal(a1, a2)
+    assert (a1 - b1).abs().max().item() < 2e-6
+
+
+# ---------------------------------------------------------------------------------------------------
+# edge cases of the ABI
+def test_nonfinite_inputs_are_isolated(oracle):
+    H = inputs.normal(64, 1.0, config=66)[0]
+    H[5, 2, 3] = np.nan
+    H[17, 0, 0] = np.inf
+    H[18, 1, 1] = -np.inf
+    for variant in (1, 2):
+        bk.birkhoff4_set_variant(variant)
+        P = gpu_forward(H)
+        bk.birkhoff4_set_variant(0)
+        for b in (5, 17, 18):
+            assert np.isnan(P[b]).all()
+        good = np.ones(64, bool)
+        good[[5, 17, 18]] = False
+        assert np.isfinite(P[good]).all()
+        assert np.abs(P[good] - oracle.forward(H[good])).max() < TOL_P
+
+
+def test_extreme_magnitudes(oracle):
+    rng = np.random.default_rng(3)
+    H = (rng.normal(size=(512, 4, 4)) * 1e4).astype(np.float32)
+    H[:8] = rng.choice([-1e4, 1e4], size=(8, 4, 4)).astype(np.float32)          # massive ties
+    H[8:16] = (rng.normal(size=(8, 4, 4)) * 1e-6).astype(np.float32)
+    P = gpu_forward(H, max_iter=64)
+    assert np.isfinite(P).all()
+    assert np.abs(P.sum(2) - 1).max() < 1e-6
+    P_o, info = oracle.forward(H.astype(np.float64), return_info=True)
+    ok = info["err"] <= oracle.CERTIFY
+    assert np.abs(P - P_o)[ok].max() < 1e-4                                      # |H| ~ 4e4: ulp(H) alone is 4e-3
+
+
+def test_max_iter_and_tol_semantics():
+    H = dev(inputs.normal(4096, 1.0, config=67)[0])
+    it = torch.zeros(4096, dtype=torch.int32, device="cuda")
+    P0 = bk.birkhoff4_forward_ex(H, max_iter=0, iters=it)
+    assert int(it.max()) == 0
+    rows = host(P0).astype(np.float64).sum(2)
+    assert np.abs(rows - 1).max() < 1e-6                                         # rows normalised even at max_iter = 0
+    for cap in (1, 2, 3):
+        bk.birkhoff4_forward_ex(H, max_iter=cap, iters=it)
+        assert int(it.max()) <= cap
+    # looser tolerance never takes more updates; tol = 0 runs to the floor and still terminates
+    it_loose, it_tight, it_zero = (torch.zeros(4096, dtype=torch.int32, device="cuda") for _ in range(3))
+    bk.birkhoff4_forward_ex(H, tol=1e-3, iters=it_loose)
+    bk.birkhoff4_forward_ex(H, tol=1e-6, iters=it_tight)
+    Pz = bk.birkhoff4_forward_ex(H, tol=0.0, max_iter=50, iters=it_zero)
+    assert bool((it_loose <= it_tight).all())
+    assert int(it_zero.max()) < 50
+    assert np.isfinite(host(Pz)).all()
+
+
+def test_diagnostics_consistent():
+    c = inputs.make(5, B=50001)
+    H = dev(c["H"])
+    it = torch.zeros(50001, dtype=torch.int32, device="cuda")
+    hist = torch.zeros(64, dtype=torch.int64, device="cuda")
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for variant in (1, 2):
+        it.zero_(), hist.zero_(), unc.zero_()
+        bk.birkhoff4_set_variant(variant)
+        P = bk.birkhoff4_forward_ex(H, max_iter=32, iters=it, hist=hist, n_unconverged=unc)
+        bk.birkhoff4_set_variant(0)
+        h = host(hist)
+        assert h.sum() == 50001
+        assert (np.bincount(np.minimum(host(it), 63), minlength=64) == h).all()
+        assert torch.equal(P, bk.birkhoff4_forward(H, max_iter=32))              # diagnostics do not change P
+        assert 0 <= int(host(unc)[0]) <= 50001
+
+
+def test_aliasing_in_place():
+    H, G = inputs.normal(5000, 1.0, config=68)
+    Hd, Gd = dev(H), dev(G)
+    P = bk.birkhoff4_forward(Hd)
+    dH = bk.birkhoff4_backward(P, Gd)
+    X = Hd.clone()
+    bk.birkhoff4_forward(X, X)                                                   # P == H
+    assert torch.equal(X, P)
+    Y = Gd.clone()
+    bk.birkhoff4_backward(P, Y, Y)                                               # dH == dP
+    assert torch.equal(Y, dH)
+
+
+def test_invalid_arguments_return_einval():
+    L = bk.lib()
+    import ctypes
+    t = torch.zeros((4, 4, 4), device="cuda")
+    p = ctypes.c_void_p(t.data_ptr())
+    mis = ctypes.c_void_p(t.data_ptr() + 4)
+    nan = float("nan")
+    assert L.birkhoff4_forward(p, p, -1, 1e-6, 20, None) == 1
+    assert L.birkhoff4_forward(None, p, 4, 1e-6, 20, None) == 1
+    assert L.birkhoff4_forward(p, None, 4, 1e-6, 20, None) == 1
+    assert L.birkhoff4_forward(mis, p, 1, 1e-6, 20, None) == 1
+    assert L.birkhoff4_forward(p, p, 4, -1.0, 20, None) == 1
+    assert L.birkhoff4_forward(p, p, 4, nan, 20, None) == 1
+    assert L.birkhoff4_forward(p, p, 4, 1e-6, -1, None) == 1
+    assert L.birkhoff4_backward(p, None, p, 4, None) == 1
+    assert L.birkhoff4_backward(p, mis, p, 1, None) == 1
+    assert L.birkhoff4_sinkhorn(p, p, 4, -1, None) == 1
+    with pytest.raises(bk.Birkhoff4Error):
+        bk.birkhoff4_forward(torch.zeros(4, 4, 4))                               # CPU tensor: no CPU path
+    with pytest.raises(bk.Birkhoff4Error):
+        bk.birkhoff4_forward(torch.zeros(4, 4, 4, device="cuda", dtype=torch.float64))
+
+
+def test_non_default_stream():
+    H, G = inputs.normal(1 << 16, 1.0, config=69)
+    Hd, Gd = dev(H), dev(G)
+    ref = bk.birkhoff4_forward(Hd)
+    ref_d = bk.birkhoff4_backward(ref, Gd)
+    torch.cuda.synchronize()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        P = bk.birkhoff4_forward(Hd)
+        dH = bk.birkhoff4_backward(P, Gd)
+    st.synchronize()
+    assert torch.equal(P, ref) and torch.equal(dH, ref_d)
+
+
+# ---------------------------------------------------------------------------------------------------
+# backward on its own: fed the oracle's P (rounded to fp32), including near-permutation P where the
+# paper's Delta is singular (S7)
+@pytest.mark.parametrize("s", [1.0, 10.0, 100.0])
+def test_backward_alone(oracle, s):
+    H, G = inputs.normal(8192, s, config=70)
+    P_o = oracle.forward(H.astype(np.float64))
+    dH = host(bk.birkhoff4_backward(dev(P_o.astype(np.float32)), dev(G))).astype(np.float64)
+    dH_o = oracle.backward(P_o, G.astype(np.float64))
+    assert np.isfinite(dH).all()
+    e1, e2 = dh_errors(dH, dH_o, G)
+    assert e1 <= TOL_DH and e2 <= TOL_DH
+    print("backward alone s=%g" % s, e1, e2)
+
+
+def test_backward_exact_permutation_and_additive_G():
+    P = np.zeros((24, 4, 4), np.float32)
+    for k, p in enumerate(itertools.permutations(range(4))):
+        P[k, np.arange(4), list(p)] = 1.0
+    G = inputs.normal(24, 1.0, config=71)[1]
+    dH = host(bk.birkhoff4_backward(dev(P), dev(G)))
+    assert np.isfinite(dH).all() and np.abs(dH).max() < 1e-5                     # a vertex: the Jacobian vanishes
+    # P12: G_ij = a_i + b_j gives dH = 0
+    Hn = inputs.normal(1024, 2.0, config=72)[0]
+    Pn = bk.birkhoff4_forward(dev(Hn))
+    rng = np.random.default_rng(5)
+    Ga = (rng.normal(size=(1024, 4, 1)) + rng.normal(size=(1024, 1, 4))).astype(np.float32)
+    assert np.abs(host(bk.birkhoff4_backward(Pn, dev(Ga)))).max() < 5e-6
+
+
+# ---------------------------------------------------------------------------------------------------
+# Sinkhorn-20 baseline kernel: same convention as the oracle's eq. (2) and as the paper's Table 2
+def test_sinkhorn_kernel_matches_oracle(oracle):
+    for s, n_iter in ((1.0, 20), (10.0, 20), (3.0, 1), (3.0, 0)):
+        H = inputs.normal(4096, s, config=73)[0]
+        T = host(bk.birkhoff4_sinkhorn(dev(H), n_iter=n_iter)).astype(np.float64)
+        T_o = oracle.sinkhorn(H.astype(np.float64), n_iter=n_iter)
+        if n_iter == 0:                                                           # K = exp(H) up to the row shift
+            T_o = T_o / T_o.max(axis=2, keepdims=True)
+            T = T / T.max(axis=2, keepdims=True)
+        assert np.abs(T - T_o).max() < 2e-5
+
+
+def test_sinkhorn20_table2_statistics(oracle):
+    import os
+    rows = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_table2_sinkhorn20.txt")) as f:
+        for line in f:
+            if not line.startswith("#") and line.strip():
+                k = line.split()
+                rows[k[0]] = (float(k[1]) * 1e-3, float(k[3]) * 1e-3)
+    H = inputs.normal(100000, 10.0, config=74)[0]
+    err = oracle.marginal_err(host(bk.birkhoff4_sinkhorn(dev(H), n_iter=20)))
+    mean, med = rows["N(0,10^2)"]
+    assert abs(err.mean() - mean) < 0.05 * mean and abs(np.median(err) - med) < 0.05 * med
+    H = inputs.uniform(100000, 10.0, config=74)[0]
+    err = oracle.marginal_err(host(bk.birkhoff4_sinkhorn(dev(H), n_iter=20)))
+    mean, med = rows["Unif(-10,10)"]
+    assert abs(err.mean() - mean) < 0.05 * mean and abs(np.median(err) - med) < 0.05 * med
+
+
+# ---------------------------------------------------------------------------------------------------
+# host-buffer entry points (the end-to-end path bench.py times): same bits as the device-pointer calls
+@pytest.mark.parametrize("B", [1, 1000, (1 << 18) + 17, (1 << 19) * 3 + 5])
+def test_host_calls_match_device_calls(B):
+    H, G = inputs.normal(B, 2.0, config=75)
+    Hd, Gd = dev(H), dev(G)
+    P = bk.birkhoff4_forward(Hd)
+    dH = bk.birkhoff4_backward(P, Gd)
+    Hh, Gh = torch.from_numpy(H).pin_memory(), torch.from_numpy(G).pin_memory()
+    Ph = bk.birkhoff4_forward_host(Hh)
+    assert torch.equal(Ph, P.cpu())
+    assert torch.equal(bk.birkhoff4_backward_host(Ph, Gh), dH.cpu())
+    P2, dH2 = bk.birkhoff4_forward_backward_host(Hh, Gh)
+    assert torch.equal(P2, P.cpu()) and torch.equal(dH2, dH.cpu())
+    _, dH3 = bk.birkhoff4_forward_backward_host(torch.from_numpy(H), torch.from_numpy(G), want_P=False)   # pageable
+    assert torch.equal(dH3, dH.cpu())
+    bk.birkhoff4_host_release()
