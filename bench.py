@@ -198,6 +198,8 @@ def run_ours(args, wl):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     bk.lib()                                                                   # raises if libbirkhoff4.so cannot be had
+    if args.variant:
+        bk.birkhoff4_set_variant(args.variant)                                 # measurement only; 0 = library default
 
     B, bf16, max_iter = wl["B"], wl["config"] == 4, wl["max_iter"]
     set_bytes = B * (32 if bf16 else 64) + 3 * B * 64
@@ -327,6 +329,7 @@ def run_ours(args, wl):
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "desc": wl["desc"], "B_per_gpu": B, "tol": TOL, "max_iter": max_iter,
+                   "variant": args.variant,
                    "parallelism": "batch shards, no collective" if world > 1 else "single GPU",
                    "l2": "rotation over %d buffer sets (%.2f GiB); backward reads the P written %d steps earlier"
                          % (nsets, nsets * set_bytes / 2 ** 30, nsets - 1)},
@@ -358,6 +361,7 @@ def main():
     ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", type=int, default=0, help="forward kernel variant (0 = library default)")
     args = ap.parse_args()
     wl = WORKLOADS[args.workload]
     if args.impl == "reference":

@@ -6,6 +6,7 @@
 // sectors and nothing is fetched twice.  All intermediates live in registers.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include <mutex>
 
@@ -84,6 +85,8 @@ BK4_DEV void load_logits(const void* H, int64_t b, float (&m)[16]) {
 // logit range (max - min over the 16 entries) above which a matrix takes the LP dual start (S1):
 // N(0,1) logits stay below it, N(0,2^2) and larger mostly exceed it.
 constexpr float kHardRange = 8.0f;
+// logit range up to which a matrix first tries the lean iteration (lean_forward); chosen by measurement, DESIGN.md
+constexpr float kEasyRange = 8.0f;
 
 struct FwdDiag {
     int32_t* iters;
@@ -160,7 +163,76 @@ __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H
                 if (!converged) atomicAdd(&s_unc, 1u);
             }
         };
-        newton_forward<V>(Hv, hardm, any_hard, tol_i, max_iter, reload, emit);
+        newton_forward<V>(Hv, hardm, any_hard, msplat(V{}, false), tol_i, max_iter, reload, emit);
+    }
+    if constexpr (DIAG) {
+        __syncthreads();
+        if (diag.hist && threadIdx.x < BIRKHOFF4_HIST_BINS && s_hist[threadIdx.x])
+            atomicAdd(&diag.hist[threadIdx.x], (unsigned long long)s_hist[threadIdx.x]);
+        if (diag.n_unconverged && threadIdx.x == 0 && s_unc) atomicAdd(diag.n_unconverged, (unsigned long long)s_unc);
+    }
+}
+
+// ---------------------------------------------------------------- forward kernel, variant 3 (default)
+// One matrix per thread.  Matrices whose logit range is at most `easy_range` run lean_forward in warp lockstep
+// and are stored together; the others (large range, NaN/Inf, or a failed lean iteration: a few per million on
+// N(0,1) logits) run the guarded newton_forward afterwards, in a branch the warp skips when it has none.
+template <bool BF16, bool DIAG, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void* __restrict__ H, float* __restrict__ P,
+                                                           int64_t B, float tol_i, int max_iter, float e_min,
+                                                           FwdDiag diag) {
+    __shared__ unsigned int s_hist[DIAG ? BIRKHOFF4_HIST_BINS : 1];
+    __shared__ unsigned int s_unc;
+    if constexpr (DIAG) {
+        if (threadIdx.x < BIRKHOFF4_HIST_BINS) s_hist[threadIdx.x] = 0;
+        if (threadIdx.x == 0) s_unc = 0;
+        __syncthreads();
+    }
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = b < B;
+    const int64_t idx = valid ? b : B - 1;  // padding lanes shadow the last matrix and store nothing
+    unsigned need_robust = valid ? 1u : 0u;
+    {
+        float h[16], T[16];
+        load_logits<BF16>(H, idx, h);
+        int iters;
+        const unsigned status = lean_forward(h, valid, e_min, tol_i, max_iter, T, iters);
+        if (valid && status != kLeanFailed) {
+            need_robust = 0u;
+            store_matrix(P + 16 * idx, T);
+            if constexpr (DIAG) {
+                if (diag.iters) diag.iters[idx] = iters;
+                atomicAdd(&s_hist[min(iters, BIRKHOFF4_HIST_BINS - 1)], 1u);
+                if (status != kLeanConverged) atomicAdd(&s_unc, 1u);
+            }
+        }
+    }
+    if (__any_sync(0xffffffffu, need_robust != 0u)) {
+        float h[16];
+        load_logits<BF16>(H, idx, h);  // the lean part has stored only matrices this branch does not touch
+        float hmax = h[0], hmin = h[0], poison = 0.0f;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            hmax = fmaxf(hmax, h[q]);
+            hmin = fminf(hmin, h[q]);
+            poison = __fmaf_rn(h[q], 0.0f, poison);  // NaN iff some logit is NaN or +-Inf (fmaxf skips NaN)
+        }
+        const bool bad = !(poison == 0.0f);
+        const bool hard = hmax - hmin > kHardRange;
+        const bool any_hard = __any_sync(0xffffffffu, need_robust != 0u && hard);
+        auto reload = [&](float(&Hr)[16]) { load_logits<BF16>(H, idx, Hr); };
+        auto emit = [&](int, const float(&T)[16], int iters, bool converged) {
+            float out[16];
+#pragma unroll
+            for (int q = 0; q < 16; ++q) out[q] = bad ? kNaN : T[q];
+            store_matrix(P + 16 * idx, out);
+            if constexpr (DIAG) {
+                if (diag.iters) diag.iters[idx] = iters;
+                atomicAdd(&s_hist[min(iters, BIRKHOFF4_HIST_BINS - 1)], 1u);
+                if (!converged) atomicAdd(&s_unc, 1u);
+            }
+        };
+        newton_forward<float>(h, bool1(hard), any_hard, bool1(need_robust == 0u), tol_i, max_iter, reload, emit);
     }
     if constexpr (DIAG) {
         __syncthreads();
@@ -195,7 +267,16 @@ __global__ void __launch_bounds__(256) sinkhorn_kernel(const float* __restrict__
 
 // ---------------------------------------------------------------- host side
 static int g_variant = 0;
-constexpr int kDefaultVariant = 1;
+constexpr int kDefaultVariant = 4;
+static float g_easy_range = -1.0f;  // < 0: kEasyRange, or BIRKHOFF4_EASY_RANGE from the environment (tuning only)
+
+static float easy_range() {
+    if (g_easy_range < 0.0f) {
+        const char* e = getenv("BIRKHOFF4_EASY_RANGE");
+        g_easy_range = e ? (float)atof(e) : kEasyRange;
+    }
+    return g_easy_range;
+}
 constexpr int kThreads = 256;
 
 static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) != 0; }
@@ -215,11 +296,24 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
     if (!H || !P || misaligned(H) || misaligned(P)) return BIRKHOFF4_EINVAL;
     const bool want_diag = diag.iters || diag.hist || diag.n_unconverged;
     const int variant = g_variant ? g_variant : kDefaultVariant;
-    const int nl = variant == 1 ? 1 : 2;
+    const int nl = variant == 2 ? 2 : 1;
     const int64_t threads = (B + nl - 1) / nl;
     const unsigned grid = (unsigned)((threads + kThreads - 1) / kThreads);
     const float tol_i = internal_tol(tol);
-    if (nl == 1) {
+    if (variant >= 3) {
+        const float em = expf(-easy_range());
+#define BK4_LAUNCH_LEAN(T, M)                                                                                     \
+    do {                                                                                                          \
+        const unsigned g = (unsigned)((B + (T)-1) / (T));                                                         \
+        if (want_diag) forward_lean_kernel<BF16, true, T, M><<<g, T, 0, stream>>>(H, P, B, tol_i, max_iter, em, diag); \
+        else forward_lean_kernel<BF16, false, T, M><<<g, T, 0, stream>>>(H, P, B, tol_i, max_iter, em, diag);     \
+    } while (0)
+        if (variant == 3) BK4_LAUNCH_LEAN(256, 3);
+        else if (variant == 4) BK4_LAUNCH_LEAN(256, 4);
+        else if (variant == 5) BK4_LAUNCH_LEAN(128, 8);
+        else BK4_LAUNCH_LEAN(128, 6);
+#undef BK4_LAUNCH_LEAN
+    } else if (nl == 1) {
         if (want_diag) forward_kernel<1, BF16, true><<<grid, kThreads, 0, stream>>>(H, P, B, tol_i, max_iter, diag);
         else forward_kernel<1, BF16, false><<<grid, kThreads, 0, stream>>>(H, P, B, tol_i, max_iter, diag);
     } else {
@@ -368,7 +462,7 @@ void birkhoff4_host_release(void) {
 
 int birkhoff4_set_variant(int variant) {
     const int old = g_variant;
-    if (variant >= 0 && variant <= 2) g_variant = variant;
+    if (variant >= 0 && variant <= 6) g_variant = variant;
     return old;
 }
 

@@ -13,6 +13,8 @@
 // (3 exponentials instead of 16), and the row-max shift mu_i keeps every exponential <= 1 as in PAPER.md:186-191.
 // When |delta| grows past 2^40 the base is moved (beta0 += delta, E recomputed from H).
 #pragma once
+#include <type_traits>
+
 #include "bk4_vec.cuh"
 
 #ifndef BK4_TRACE  // development hook (host emulation of the solver); compiles to nothing in the library
@@ -248,9 +250,12 @@ BK4_DEV void lp_dual_start(const V (&H)[16], V (&b0)[3]) {
 // `any_hard` must be uniform over the threads that execute together (it only selects the cheaper start-up
 // code when no matrix needs the LP start).  Reload(H) re-reads the logits (used when the base point moves);
 // Emit(half, T, iters, converged) receives the result of one matrix as soon as it is final.
+// `skip` marks matrices this call must leave alone (already finished by lean_forward, or padding): they start out
+// `done`, nothing is emitted for them and their arithmetic is ignored.
 template <class V, class Reload, class Emit>
-BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bool any_hard, float tol_i,
-                            int max_iter, Reload&& reload, Emit&& emit) {
+BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bool any_hard,
+                            typename vtraits<V>::mask skip, float tol_i, int max_iter, Reload&& reload,
+                            Emit&& emit) {
     using M = typename vtraits<V>::mask;
     constexpr int NL = vtraits<V>::lanes;
     const V one = vsplat(V{}, 1.0f), zero = vsplat(V{}, 0.0f);
@@ -274,7 +279,7 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
 
     V vprev[3] = {v[0], v[1], v[2]};
     V errprev = vsplat(V{}, kInf);
-    M newton_trial = msplat(V{}, false), sink_trial = msplat(V{}, false), done = msplat(V{}, false);
+    M newton_trial = msplat(V{}, false), sink_trial = msplat(V{}, false), done = skip;
     int it[NL];
 #pragma unroll
     for (int k = 0; k < NL; ++k) it[k] = 0;
@@ -356,6 +361,160 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
 #pragma unroll
         for (int k = 0; k < NL; ++k) it[k] += mget(act, k) ? 1 : 0;
     }
+}
+
+// -------------------------------------------------------------------------------------------------
+// Lean Newton for well-scaled logits (one matrix per thread, the whole warp in lockstep).
+//
+// Same iteration as newton_forward -- eq. (10) for T, eq. (11) for g, the Laplacian form of eq. (12) for the
+// direction, start beta0 = 0 plus one Sinkhorn column step (S1) -- with the guard of DESIGN.md S2 reduced
+// to its test: a step after which the column residual did not fall ends the lean iteration for that matrix,
+// which is then (status kLeanFailed) solved from scratch by newton_forward, whose guard can go back and take
+// Sinkhorn steps.  On logits of small range that happens for a handful of matrices per million, so the common
+// path carries no trial/rollback state, no re-basing and no per-lane stores: a finished lane freezes its v and
+// keeps re-evaluating the same T until the warp is through, and the caller stores all results at once.
+//
+//   returns   kLeanConverged, kLeanStopped (max_iter reached, or the residual stalled at the fp32 floor:
+//             result valid, counted as unconverged) or kLeanFailed (T is not a result)
+constexpr unsigned kLeanConverged = 0u, kLeanStopped = 1u, kLeanFailed = 2u;
+constexpr float kLeanFloor = 1e-5f;  // a residual that stalls below this is the fp32 floor, not a failure
+constexpr float kLeanFloorTol = 2e-7f;  // internal tolerances below this are below the fp32 floor of the residual
+constexpr int kLeanSweeps = 3;       // start-up Sinkhorn column steps
+constexpr int kLeanFree = 2;         // Newton updates taken before the first residual test
+
+//   active    lanes holding a matrix (the others only follow the warp's votes)
+//   e_min     a matrix takes part iff every E_ij = exp(H_ij - max_k H_ik) >= e_min, i.e. its largest in-row logit
+//             range is at most -ln(e_min); the others return kLeanFailed at once (a NaN logit slips through this
+//             test, fails the first residual test and ends up in newton_forward too, which reports it)
+BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float e_min, float tol_i, int max_iter,
+                              float (&T)[16], int& iters) {
+    float E[16];
+    // E_ij = exp(H_ij - max_j H_ij): eq. (10) at beta = 0
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float m = fmaxf(fmaxf(H[4 * i], H[4 * i + 1]), fmaxf(H[4 * i + 2], H[4 * i + 3]));
+        const float t = m * -kLog2e;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) E[4 * i + j] = ex2_approx(fmaf(H[4 * i + j], kLog2e, t));
+    }
+    {
+        float lo = fminf(fminf(E[0], E[1]), E[2]);
+#pragma unroll
+        for (int q = 3; q < 15; q += 2) lo = fminf(fminf(lo, E[q]), E[q + 1]);
+        lo = fminf(lo, E[15]);
+        active = active && lo >= e_min;
+    }
+    iters = 0;
+    if (!__any_sync(0xffffffffu, active)) return kLeanFailed;
+    // start-up: kLeanSweeps Sinkhorn column steps from beta = 0 (eq. (6) PAPER.md:108 with the gauge beta_4 = 0;
+    // rows are normalised inside each step, eq. (5)): v_j *= c_4 / c_j.  Each costs a third of a Newton update and
+    // cuts the residual about 4x on N(0,1) logits, which is what lets the second Newton update land below 1e-6
+    // for 99 % of the matrices instead of 50 % (S1).
+    float v0, v1, v2;
+    {
+        float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float r = rcp_approx((E[4 * i] + E[4 * i + 1]) + (E[4 * i + 2] + E[4 * i + 3]));
+            c0 = fmaf(E[4 * i], r, c0);
+            c1 = fmaf(E[4 * i + 1], r, c1);
+            c2 = fmaf(E[4 * i + 2], r, c2);
+            c3 = fmaf(E[4 * i + 3], r, c3);
+        }
+        v0 = c3 * rcp_approx(c0);
+        v1 = c3 * rcp_approx(c1);
+        v2 = c3 * rcp_approx(c2);
+    }
+#pragma unroll
+    for (int k = 1; k < kLeanSweeps; ++k) {
+        float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float x0 = E[4 * i] * v0, x1 = E[4 * i + 1] * v1, x2 = E[4 * i + 2] * v2, x3 = E[4 * i + 3];
+            const float r = rcp_approx((x0 + x1) + (x2 + x3));
+            c0 = fmaf(x0, r, c0);
+            c1 = fmaf(x1, r, c1);
+            c2 = fmaf(x2, r, c2);
+            c3 = fmaf(x3, r, c3);
+        }
+        v0 *= c3 * rcp_approx(c0);
+        v1 *= c3 * rcp_approx(c1);
+        v2 *= c3 * rcp_approx(c2);
+    }
+    // T(beta) of eq. (10) and g_j = c_j - 1 of eq. (11), accumulated from -1 so that the partial sums stay below 1
+    // in magnitude (S9).  REFINE: one Newton-Raphson refinement of the SFU reciprocal, so that the rows
+    // of a T that may be the result sum to 1 within rounding.
+    float g0, g1, g2, g3;
+    auto eval = [&](auto refine) {
+        constexpr bool kRefine = decltype(refine)::value;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float x0 = E[4 * i] * v0, x1 = E[4 * i + 1] * v1, x2 = E[4 * i + 2] * v2, x3 = E[4 * i + 3];
+            const float s = (x0 + x1) + (x2 + x3);
+            float r = rcp_approx(s);
+            if constexpr (kRefine) r = fmaf(r, fmaf(-s, r, 1.0f), r);
+            T[4 * i] = x0 * r;
+            T[4 * i + 1] = x1 * r;
+            T[4 * i + 2] = x2 * r;
+            T[4 * i + 3] = x3 * r;
+        }
+        if constexpr (kRefine) {
+            // tested residual: two half sums, each started from -1/2, keep every partial sum below 1/2
+            g0 = ((T[0] - 0.5f) + T[4]) + ((T[8] - 0.5f) + T[12]);
+            g1 = ((T[1] - 0.5f) + T[5]) + ((T[9] - 0.5f) + T[13]);
+            g2 = ((T[2] - 0.5f) + T[6]) + ((T[10] - 0.5f) + T[14]);
+            g3 = ((T[3] - 0.5f) + T[7]) + ((T[11] - 0.5f) + T[15]);
+        } else {
+            g0 = (((T[0] - 1.0f) + T[4]) + T[8]) + T[12];
+            g1 = (((T[1] - 1.0f) + T[5]) + T[9]) + T[13];
+            g2 = (((T[2] - 1.0f) + T[6]) + T[10]) + T[14];
+            g3 = 0.0f;
+        }
+    };
+    // Newton direction (eq. (12) through the Laplacian form, S7; no ground regularisation: every T_ij of
+    // a matrix that got here is bounded away from 0) and update beta += d  <=>  v *= exp(d)
+    float d1, d2, d3;
+    auto direction = [&]() {
+        solve_grounded_laplacian<float>(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), col_dot(T, 0, 3),
+                                        col_dot(T, 1, 3), col_dot(T, 2, 3), g0, g1, g2, 0.0f, d1, d2, d3);
+    };
+    // the first kLeanFree updates are taken without looking at the residual: on these inputs no matrix is done
+    // before them, and whatever they produce is judged by the tested iterations below
+    const int n_free = max_iter < kLeanFree ? max_iter : kLeanFree;
+    for (int k = 0; k < n_free; ++k) {
+        eval(std::false_type{});
+        direction();
+        v0 *= ex2_approx(d1 * kLog2e);
+        v1 *= ex2_approx(d2 * kLog2e);
+        v2 *= ex2_approx(d3 * kLog2e);
+    }
+    float errprev = kInf;
+    unsigned running = active ? 1u : 0u, status = kLeanFailed;
+    int it = n_free;
+    for (;;) {
+        eval(std::true_type{});
+        const float err = (fabsf(g0) + fabsf(g1)) + (fabsf(g2) + fabsf(g3));
+        const bool conv = err <= tol_i;  // false for NaN: a NaN ends up in newton_forward
+        const bool improved = err < errprev;
+        if (running && (conv || !improved || it >= max_iter)) {
+            running = 0u;
+            // a residual that no longer falls: the fp32 floor if the caller asked for less than fp32 can give,
+            // otherwise newton_forward's Sinkhorn steps may still get below tol
+            status = conv ? kLeanConverged
+                          : (improved || (errprev < kLeanFloor && tol_i < kLeanFloorTol)) ? kLeanStopped : kLeanFailed;
+        }
+        if (!__any_sync(0xffffffffu, running != 0u)) break;
+        direction();
+        if (running) {  // a finished lane keeps its v (and so its T)
+            v0 *= ex2_approx(d1 * kLog2e);
+            v1 *= ex2_approx(d2 * kLog2e);
+            v2 *= ex2_approx(d3 * kLog2e);
+            errprev = err;
+            ++it;
+        }
+    }
+    iters = it;
+    return status;
 }
 
 // -------------------------------------------------------------------------------------------------
