@@ -94,12 +94,48 @@ struct FwdDiag {
     unsigned long long* n_unconverged;
 };
 
+// ---------------------------------------------------------------- launch with programmatic dependent launch
+// Every kernel of the library starts with pdl_wait() (griddepcontrol.wait: returns once the kernel before it in
+// the stream has completed and its writes are visible) and then lets the kernel after it begin launching
+// (griddepcontrol.launch_dependents).  Launched with programmatic stream serialization, the next kernel's launch
+// latency and block ramp-up overlap this kernel's tail; stream-order semantics are unchanged because nothing is
+// read or written before the wait.  BIRKHOFF4_NO_PDL=1 in the environment turns the attribute off (measurement).
+BK4_DEV void pdl_wait_and_trigger() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
+static bool use_pdl() {
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("BIRKHOFF4_NO_PDL");
+        v = (e && e[0] == '1') ? 0 : 1;
+    }
+    return v != 0;
+}
+
+template <class... KArgs, class... Args>
+static cudaError_t launch(void (*kernel)(KArgs...), unsigned grid, unsigned block, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = use_pdl() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---------------------------------------------------------------- forward kernel
 // NL = matrices per thread (1: scalar FP32, 2: packed FP32x2).
 template <int NL, bool BF16, bool DIAG>
 __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H, float* __restrict__ P, int64_t B,
                                                       float tol_i, int max_iter, FwdDiag diag) {
     using V = typename std::conditional<NL == 1, float, float2>::type;
+    pdl_wait_and_trigger();
     __shared__ unsigned int s_hist[DIAG ? BIRKHOFF4_HIST_BINS : 1];
     __shared__ unsigned int s_unc;
     if constexpr (DIAG) {
@@ -181,6 +217,7 @@ template <bool BF16, bool DIAG, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void* __restrict__ H, float* __restrict__ P,
                                                            int64_t B, float tol_i, int max_iter, float e_min,
                                                            FwdDiag diag) {
+    pdl_wait_and_trigger();
     __shared__ unsigned int s_hist[DIAG ? BIRKHOFF4_HIST_BINS : 1];
     __shared__ unsigned int s_unc;
     if constexpr (DIAG) {
@@ -245,6 +282,7 @@ __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void*
 // ---------------------------------------------------------------- backward kernel (HBM-bound: 192 B per matrix)
 __global__ void __launch_bounds__(256) backward_kernel(const float* __restrict__ P, const float* __restrict__ dP,
                                                        float* __restrict__ dH, int64_t B) {
+    pdl_wait_and_trigger();
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     float p[16], g[16], d[16];
@@ -257,6 +295,7 @@ __global__ void __launch_bounds__(256) backward_kernel(const float* __restrict__
 // ---------------------------------------------------------------- Sinkhorn-Knopp baseline kernel
 __global__ void __launch_bounds__(256) sinkhorn_kernel(const float* __restrict__ H, float* __restrict__ P, int64_t B,
                                                        int n_iter) {
+    pdl_wait_and_trigger();
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     float h[16], t[16];
@@ -300,13 +339,14 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
     const int64_t threads = (B + nl - 1) / nl;
     const unsigned grid = (unsigned)((threads + kThreads - 1) / kThreads);
     const float tol_i = internal_tol(tol);
+    cudaError_t rc = cudaSuccess;
     if (variant >= 3) {
         const float em = expf(-easy_range());
 #define BK4_LAUNCH_LEAN(T, M)                                                                                     \
     do {                                                                                                          \
         const unsigned g = (unsigned)((B + (T)-1) / (T));                                                         \
-        if (want_diag) forward_lean_kernel<BF16, true, T, M><<<g, T, 0, stream>>>(H, P, B, tol_i, max_iter, em, diag); \
-        else forward_lean_kernel<BF16, false, T, M><<<g, T, 0, stream>>>(H, P, B, tol_i, max_iter, em, diag);     \
+        if (want_diag) rc = launch(forward_lean_kernel<BF16, true, T, M>, g, T, stream, H, P, B, tol_i, max_iter, em, diag); \
+        else rc = launch(forward_lean_kernel<BF16, false, T, M>, g, T, stream, H, P, B, tol_i, max_iter, em, diag);     \
     } while (0)
         if (variant == 3) BK4_LAUNCH_LEAN(256, 3);
         else if (variant == 4) BK4_LAUNCH_LEAN(256, 4);
@@ -314,13 +354,13 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
         else BK4_LAUNCH_LEAN(128, 6);
 #undef BK4_LAUNCH_LEAN
     } else if (nl == 1) {
-        if (want_diag) forward_kernel<1, BF16, true><<<grid, kThreads, 0, stream>>>(H, P, B, tol_i, max_iter, diag);
-        else forward_kernel<1, BF16, false><<<grid, kThreads, 0, stream>>>(H, P, B, tol_i, max_iter, diag);
+        if (want_diag) rc = launch(forward_kernel<1, BF16, true>, grid, kThreads, stream, H, P, B, tol_i, max_iter, diag);
+        else rc = launch(forward_kernel<1, BF16, false>, grid, kThreads, stream, H, P, B, tol_i, max_iter, diag);
     } else {
-        if (want_diag) forward_kernel<2, BF16, true><<<grid, kThreads, 0, stream>>>(H, P, B, tol_i, max_iter, diag);
-        else forward_kernel<2, BF16, false><<<grid, kThreads, 0, stream>>>(H, P, B, tol_i, max_iter, diag);
+        if (want_diag) rc = launch(forward_kernel<2, BF16, true>, grid, kThreads, stream, H, P, B, tol_i, max_iter, diag);
+        else rc = launch(forward_kernel<2, BF16, false>, grid, kThreads, stream, H, P, B, tol_i, max_iter, diag);
     }
-    return cuda_rc(cudaGetLastError());
+    return cuda_rc(rc);
 }
 
 // ---- host-buffer path: a ring of device buffers and streams; chunked H2D -> kernels -> D2H
@@ -429,8 +469,7 @@ int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, bi
     if (B == 0) return BIRKHOFF4_OK;
     if (!P || !dP || !dH || misaligned(P) || misaligned(dP) || misaligned(dH)) return BIRKHOFF4_EINVAL;
     const unsigned grid = (unsigned)((B + kThreads - 1) / kThreads);
-    backward_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(P, dP, dH, B);
-    return cuda_rc(cudaGetLastError());
+    return cuda_rc(launch(backward_kernel, grid, kThreads, (cudaStream_t)stream, P, dP, dH, B));
 }
 
 int birkhoff4_sinkhorn(const float* H, float* P, int64_t B, int n_iter, birkhoff4_stream_t stream) {
@@ -438,8 +477,7 @@ int birkhoff4_sinkhorn(const float* H, float* P, int64_t B, int n_iter, birkhoff
     if (B == 0) return BIRKHOFF4_OK;
     if (!H || !P || misaligned(H) || misaligned(P)) return BIRKHOFF4_EINVAL;
     const unsigned grid = (unsigned)((B + kThreads - 1) / kThreads);
-    sinkhorn_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(H, P, B, n_iter);
-    return cuda_rc(cudaGetLastError());
+    return cuda_rc(launch(sinkhorn_kernel, grid, kThreads, (cudaStream_t)stream, H, P, B, n_iter));
 }
 
 int birkhoff4_forward_host(const float* H_host, float* P_host, int64_t B, float tol, int max_iter) {
