@@ -86,7 +86,7 @@ BK4_DEV void load_logits(const void* H, int64_t b, float (&m)[16]) {
 // N(0,1) logits stay below it, N(0,2^2) and larger mostly exceed it.
 constexpr float kHardRange = 8.0f;
 // logit range up to which a matrix first tries the lean iteration (lean_forward); chosen by measurement, DESIGN.md
-constexpr float kEasyRange = 8.0f;
+constexpr float kEasyRange = 12.0f;
 
 struct FwdDiag {
     int32_t* iters;
