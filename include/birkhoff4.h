@@ -56,8 +56,11 @@ typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
  *             against an internal threshold min(tol, max(tol/2, tol - 5e-7)) that leaves room for the
  *             fp32 rounding of the rows (S3/S9).  tol = 0 runs to the fp32 floor.
  *   max_iter  maximum number of updates of beta per matrix (Newton steps plus fallback column
- *             steps; PAPER.md:319 uses 20).  Function evaluations <= max_iter + 2 (one extra
- *             for the start-up column step, S1).
+ *             steps; PAPER.md:319 uses 20).  The start-up Sinkhorn column steps (three for
+ *             well-scaled logits, one after the LP start otherwise; S1) are not counted:
+ *             function evaluations <= max_iter + 4.  On well-scaled logits the first
+ *             min(2, max_iter) updates are taken without testing the residual, so a matrix reports
+ *             at least that many updates.
  * A matrix that has not converged after max_iter updates gets its last iterate (rows still
  * normalised); this is not an error (Table 2 reports such iterates too).
  */
@@ -112,7 +115,14 @@ int birkhoff4_forward_backward_host(const float* H_host, const float* dP_host, f
                                     int64_t B, float tol, int max_iter);
 void birkhoff4_host_release(void);
 
-/* Select the forward kernel variant (for measurement): 0 = library default.  Returns the previous value. */
+/*
+ * Select the forward kernel variant (for measurement).  Returns the previous value.
+ *   0  library default (= 4)
+ *   1  guarded solver for every matrix, one matrix per thread
+ *   2  guarded solver for every matrix, two matrices per thread (packed FFMA2/FADD2/FMUL2)
+ *   3  lean iteration for well-scaled logits + guarded solver for the rest, 3 blocks of 256 threads per SM
+ *   4  the same with 4 blocks per SM (64 registers)
+ */
 int birkhoff4_set_variant(int variant);
 
 const char* birkhoff4_strerror(int code);

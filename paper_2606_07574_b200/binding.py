@@ -162,7 +162,8 @@ def birkhoff4_host_release():
 
 
 def birkhoff4_set_variant(variant):
-    """0 = default; 1 = one matrix per thread (scalar FP32); 2 = two per thread (packed FP32x2)"""
+    """0 = default (4); 1/2 = guarded solver for every matrix, one/two matrices per thread; 3/4 = lean iteration
+    for well-scaled logits + guarded solver for the rest, 3/4 blocks per SM (include/birkhoff4.h)"""
     return lib().birkhoff4_set_variant(int(variant))
 
 

@@ -1,9 +1,9 @@
 // birkhoff4.cu -- kernels and C ABI of libbirkhoff4.so (include/birkhoff4.h).  sm_100a only.
 //
-// Mapping: one thread owns one matrix (variant 1, scalar FP32) or two adjacent matrices (variant 2, every
-// FP32 instruction a packed FFMA2/FADD2/FMUL2).  A 64-byte matrix is two 32-byte DRAM sectors, so each thread
-// moves its matrix with 256-bit LDG/STG (ld.global.v8.f32, new on sm_100): every request touches whole
-// sectors and nothing is fetched twice.  All intermediates live in registers.
+// Mapping: one thread owns one matrix (two adjacent matrices in variant 2, where every FP32 instruction is a
+// packed FFMA2/FADD2/FMUL2).  A 64-byte matrix is two 32-byte DRAM sectors, so each thread moves its matrix with
+// 256-bit LDG/STG (ld.global.v8.f32, new on sm_100): every request touches whole sectors and nothing is fetched
+// twice.  All intermediates live in registers.  Variants: include/birkhoff4.h.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -209,10 +209,11 @@ __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H
     }
 }
 
-// ---------------------------------------------------------------- forward kernel, variant 3 (default)
-// One matrix per thread.  Matrices whose logit range is at most `easy_range` run lean_forward in warp lockstep
-// and are stored together; the others (large range, NaN/Inf, or a failed lean iteration: a few per million on
-// N(0,1) logits) run the guarded newton_forward afterwards, in a branch the warp skips when it has none.
+// ---------------------------------------------------------------- forward kernel, variants 3 and 4 (default)
+// One matrix per thread.  Matrices whose largest in-row logit range is at most -ln(e_min) run lean_forward in warp
+// lockstep and are stored together; the others (large range, NaN/Inf, or a failed lean iteration: none in a
+// million N(0,1) matrices) run the guarded newton_forward afterwards, in a branch the warp skips when it has none.
+// A matrix's result depends on that matrix alone, not on which matrices share its warp.
 template <bool BF16, bool DIAG, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void* __restrict__ H, float* __restrict__ P,
                                                            int64_t B, float tol_i, int max_iter, float e_min,
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void*
                 if (!converged) atomicAdd(&s_unc, 1u);
             }
         };
-        newton_forward<float>(h, bool1(hard), any_hard, bool1(need_robust == 0u), tol_i, max_iter, reload, emit);
+        newton_forward<float, true>(h, bool1(hard), any_hard, bool1(need_robust == 0u), tol_i, max_iter, reload, emit);
     }
     if constexpr (DIAG) {
         __syncthreads();
@@ -349,9 +350,7 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
         else rc = launch(forward_lean_kernel<BF16, false, T, M>, g, T, stream, H, P, B, tol_i, max_iter, em, diag);     \
     } while (0)
         if (variant == 3) BK4_LAUNCH_LEAN(256, 3);
-        else if (variant == 4) BK4_LAUNCH_LEAN(256, 4);
-        else if (variant == 5) BK4_LAUNCH_LEAN(128, 8);
-        else BK4_LAUNCH_LEAN(128, 6);
+        else BK4_LAUNCH_LEAN(256, 4);
 #undef BK4_LAUNCH_LEAN
     } else if (nl == 1) {
         if (want_diag) rc = launch(forward_kernel<1, BF16, true>, grid, kThreads, stream, H, P, B, tol_i, max_iter, diag);
@@ -500,7 +499,7 @@ void birkhoff4_host_release(void) {
 
 int birkhoff4_set_variant(int variant) {
     const int old = g_variant;
-    if (variant >= 0 && variant <= 6) g_variant = variant;
+    if (variant >= 0 && variant <= 4) g_variant = variant;
     return old;
 }
 

@@ -252,7 +252,9 @@ BK4_DEV void lp_dual_start(const V (&H)[16], V (&b0)[3]) {
 // Emit(half, T, iters, converged) receives the result of one matrix as soon as it is final.
 // `skip` marks matrices this call must leave alone (already finished by lean_forward, or padding): they start out
 // `done`, nothing is emitted for them and their arithmetic is ignored.
-template <class V, class Reload, class Emit>
+// LANE_INDEPENDENT: a matrix's arithmetic does not depend on which other matrices share its warp (the cheaper
+// start-up code for warps without a `hard` matrix rounds differently), at the cost of a few instructions.
+template <class V, bool LANE_INDEPENDENT = false, class Reload, class Emit>
 BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bool any_hard,
                             typename vtraits<V>::mask skip, float tol_i, int max_iter, Reload&& reload,
                             Emit&& emit) {
@@ -269,7 +271,7 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
         for (int j = 0; j < 3; ++j) b0[j] = vsel(hard, bl[j], zero);
         base_exponentials(H, b0, false, E);
     } else {
-        base_exponentials(H, b0, true, E);
+        base_exponentials(H, b0, !LANE_INDEPENDENT, E);
     }
 
     // start-up column step (v = 1): v_j = c_4 / c_j

@@ -65,7 +65,7 @@ def check_forward_backward(oracle, H32, G32, H_for_oracle=None, P_gpu=None, err_
 
 # ---------------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json configs[0]): B = 1024, N(0,1), every element against the oracle
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 def test_config1_full_parity(oracle, variant):
     c = inputs.make(1)
     old = bk.birkhoff4_set_variant(variant)
@@ -77,7 +77,7 @@ def test_config1_full_parity(oracle, variant):
 
 
 # several tiles and a ragged tail, both thread mappings
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 4])
 @pytest.mark.parametrize("B", [1, 2, 3, 31, 33, 255, 257, 1000, 4097, 70001])
 def test_ragged_sizes(oracle, variant, B):
     H, G = inputs.normal(B, 1.0, config=60, sub=B)
@@ -105,7 +105,7 @@ def test_empty_batch():
 
 
 # the paper's distributions (Tables 1-2) and the larger scales of config 3
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 4])
 @pytest.mark.parametrize("s", [0.1, 1.0, 2.0, 3.0, 5.0, 10.0, 30.0, 100.0])
 def test_scales_parity(oracle, s, variant):
     H, G = inputs.normal(8192, s, config=61)
@@ -137,7 +137,7 @@ def test_config4_bf16_small(oracle):
 
 
 # config 5: heterogeneous structure (near-permutations, duplicate rows, ties, scales 0.1..100)
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 def test_config5_small(oracle, variant):
     c = inputs.make(5, B=16384 + 7)
     old = bk.birkhoff4_set_variant(variant)
@@ -262,6 +262,77 @@ def test_two_variants_agree_and_deterministic():
     assert (a1 - b1).abs().max().item() < 2e-6
 
 
+def _mixed_batch(n=4096, seed=71):
+    """well-scaled, large-range, row-offset, near-permutation and NaN matrices interleaved inside every warp"""
+    rng = np.random.default_rng(seed)
+    H = rng.normal(size=(n, 4, 4)).astype(np.float32)
+    k = np.arange(n) % 8
+    H[k == 1] *= 30.0                                                            # guarded solver, LP start
+    H[k == 2] += (rng.normal(size=(n, 4, 1)) * 50).astype(np.float32)[k == 2]    # huge row offsets, small in-row range
+    H[k == 3] *= 6.0                                                             # in-row range around the lean limit
+    idx = np.nonzero(k == 4)[0]
+    for i in range(4):
+        H[idx, i, (i + idx) % 4] += 9.0                                          # near-permutation
+    H[k == 5] += (rng.normal(size=(n, 1, 4)) * 50).astype(np.float32)[k == 5]    # huge column offsets
+    return H
+
+
+def test_lean_and_guarded_matrices_share_warps(oracle):
+    H = _mixed_batch()
+    G = np.random.default_rng(72).normal(size=H.shape).astype(np.float32)
+    r = check_forward_backward(oracle, H, G, err_gate=3e-6, max_iter=32)
+    print("mixed warps", r)
+    Hn = H.copy()
+    Hn[7::64, 1, 2] = np.nan                                                     # one NaN matrix in every other warp
+    P = gpu_forward(Hn, max_iter=32)
+    bad = np.zeros(len(H), bool)
+    bad[7::64] = True
+    assert np.isnan(P[bad]).all() and np.isfinite(P[~bad]).all()
+    assert np.abs(P[~bad] - gpu_forward(H, max_iter=32)[~bad]).max() == 0.0      # neighbours of a NaN are untouched
+
+
+def test_result_depends_on_the_matrix_alone():
+    """default kernel: permuting the batch permutes the output bit for bit (no dependence on warp neighbours)"""
+    H = _mixed_batch(8192, seed=73)
+    P = gpu_forward(H, max_iter=32)
+    perm = np.random.default_rng(74).permutation(len(H))
+    Pp = gpu_forward(H[perm], max_iter=32)
+    assert np.array_equal(Pp, P[perm])
+    assert np.array_equal(gpu_forward(H[:1000], max_iter=32), P[:1000])          # and so does truncating it
+    assert np.array_equal(gpu_forward(H, max_iter=32), P)                        # deterministic
+
+
+def test_all_variants_agree():
+    H = dev(_mixed_batch(1 << 15, seed=75))
+    out = []
+    for variant in (1, 2, 3, 4):
+        bk.birkhoff4_set_variant(variant)
+        out.append(bk.birkhoff4_forward(H, max_iter=32))
+        bk.birkhoff4_set_variant(0)
+    assert torch.equal(out[2], out[3])                                           # 3 and 4 differ in launch bounds only
+    for o in out[1:]:
+        assert (o - out[0]).abs().max().item() < 3e-6
+
+
+def test_lean_iteration_counts_and_floor():
+    """well-scaled logits: two untested updates, then tested ones; tol = 0 stops at the fp32 floor"""
+    H = dev(inputs.normal(1 << 14, 1.0, config=76)[0])
+    it = torch.zeros(1 << 14, dtype=torch.int32, device="cuda")
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    P = bk.birkhoff4_forward_ex(H, iters=it, n_unconverged=unc)
+    assert int(it.min()) == 2 and int(it.max()) <= 4 and int(unc.item()) == 0
+    assert float(it.float().mean()) < 2.1
+    it1 = torch.zeros_like(it)
+    P1 = bk.birkhoff4_forward_ex(H, max_iter=1, iters=it1)
+    assert int(it1.max()) == 1 and int(it1.min()) == 1
+    unc.zero_()
+    Pz = bk.birkhoff4_forward_ex(H, tol=0.0, max_iter=50, iters=it, n_unconverged=unc)
+    assert int(it.max()) < 12 and int(unc.item()) > 0.99 * (1 << 14)             # (almost) nobody computes Err = 0: they stop at the floor
+    assert (Pz - P).abs().max().item() < 5e-7
+    rows = host(P1).astype(np.float64).sum(2)
+    assert np.abs(rows - 1).max() < 1e-6
+
+
 # ---------------------------------------------------------------------------------------------------
 # edge cases of the ABI
 def test_nonfinite_inputs_are_isolated(oracle):
@@ -269,7 +340,7 @@ def test_nonfinite_inputs_are_isolated(oracle):
     H[5, 2, 3] = np.nan
     H[17, 0, 0] = np.inf
     H[18, 1, 1] = -np.inf
-    for variant in (1, 2):
+    for variant in (1, 2, 4):
         bk.birkhoff4_set_variant(variant)
         P = gpu_forward(H)
         bk.birkhoff4_set_variant(0)
@@ -320,7 +391,7 @@ def test_diagnostics_consistent():
     it = torch.zeros(50001, dtype=torch.int32, device="cuda")
     hist = torch.zeros(64, dtype=torch.int64, device="cuda")
     unc = torch.zeros(1, dtype=torch.int64, device="cuda")
-    for variant in (1, 2):
+    for variant in (1, 2, 4):
         it.zero_(), hist.zero_(), unc.zero_()
         bk.birkhoff4_set_variant(variant)
         P = bk.birkhoff4_forward_ex(H, max_iter=32, iters=it, hist=hist, n_unconverged=unc)
