@@ -16,9 +16,12 @@ runs forward on set i % sets and backward on set (i+1) % sets, whose P was writt
 backward reads P from HBM as it does in training, where the rest of the network runs in between.
 
 One JSON line on stdout (rank 0).  `value` = matrices/s through forward+backward with inputs resident in HBM
-(CUDA events on the launching stream, max over ranks); `e2e` = the same through the host-buffer C-ABI call
-birkhoff4_forward_backward_host (pinned host memory in, P and dH back out, copies inside the timed region);
-`roofline` = the slower kernel of the step against the measured HBM copy bandwidth (MEASURED_PEAKS.json);
+(K steps between two CUDA events on the launching stream, max over ranks); `e2e` = the same through the
+host-buffer C-ABI call birkhoff4_forward_backward_host (pinned host memory in, P and dH back out, copies inside
+the timed region); `roofline_kernels` = each kernel's average launch duration (K back-to-back launches of that
+kernel over the same rotation between two events) against the measured HBM copy bandwidth (MEASURED_PEAKS.json),
+`roofline` = the slower of the two, `traffic` = ncu DRAM bytes per launch from profiles/traffic.csv;
+`fwd.update_histogram` = share of matrices by number of Newton updates (BASELINE.json configs[2] asks for it);
 `cpu_baseline` = the fp64 oracle timed on this host on a bounded sample (a reported baseline, not the target).
 `--impl reference` times that oracle alone (rank 0 only); the oracle is test infrastructure and is imported
 nowhere else in this file's GPU path.
@@ -273,6 +276,7 @@ def run_ours(args, wl):
         bk.birkhoff4_forward_ex(sets[0]["H"], sets[0]["P"], TOL, max_iter, hist=hist, n_unconverged=unc)
     h = hist.cpu().numpy()
     mean_updates = float((h * np.arange(64)).sum() / max(h.sum(), 1)) if not bf16 else None
+    update_hist = {str(k): round(float(h[k]) / max(h.sum(), 1), 6) for k in range(64) if h[k]} if not bf16 else None
     del P64, err
 
     # ---- Sinkhorn-20 baseline kernel of the same library (context: PAPER.md:32, 319), fp32 workloads only
@@ -341,6 +345,7 @@ def run_ours(args, wl):
                    "l2": "rotation over %d buffer sets (%.2f GiB); backward reads the P written %d steps earlier"
                          % (nsets, nsets * set_bytes / 2 ** 30, nsets - 1)},
         "fwd": {"value": world * B / (f_ms * 1e-3), "unit": UNIT, "mean_newton_updates": mean_updates,
+                "update_histogram": update_hist,
                 "unconverged": int(unc.item())},
         "max_marginal_err": max_err, "mean_marginal_err": mean_err,
         "roofline": roofline, "roofline_kernels": kernels, "sinkhorn20_gpu": sink,

@@ -85,7 +85,8 @@ BK4_DEV void load_logits(const void* H, int64_t b, float (&m)[16]) {
 // logit range (max - min over the 16 entries) above which a matrix takes the LP dual start (S1):
 // N(0,1) logits stay below it, N(0,2^2) and larger mostly exceed it.
 constexpr float kHardRange = 8.0f;
-// logit range up to which a matrix first tries the lean iteration (lean_forward); chosen by measurement, DESIGN.md
+// largest in-row logit range up to which lean_forward starts from beta = 0 (above: LP dual start); chosen by
+// measurement, DESIGN.md
 constexpr float kEasyRange = 12.0f;
 
 struct FwdDiag {
@@ -210,13 +211,14 @@ __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H
 }
 
 // ---------------------------------------------------------------- forward kernel, variants 3 and 4 (default)
-// One matrix per thread.  Matrices whose largest in-row logit range is at most -ln(e_min) run lean_forward in warp
-// lockstep and are stored together; the others (large range, NaN/Inf, or a failed lean iteration: none in a
-// million N(0,1) matrices) run the guarded newton_forward afterwards, in a branch the warp skips when it has none.
+// One matrix per thread.  Every matrix first runs lean_forward in warp lockstep (LP dual start when its largest
+// in-row logit range exceeds lp_range) and the results are stored together; what that leaves (NaN/Inf, or a lean
+// iteration whose residual stopped falling: none in a million N(0,1) matrices, about one in a thousand at
+// N(0,30^2)) runs the guarded newton_forward afterwards, in a branch the warp skips when it has none.
 // A matrix's result depends on that matrix alone, not on which matrices share its warp.
 template <bool BF16, bool DIAG, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void* __restrict__ H, float* __restrict__ P,
-                                                           int64_t B, float tol_i, int max_iter, float e_min,
+                                                           int64_t B, float tol_i, int max_iter, float lp_range,
                                                            FwdDiag diag) {
     pdl_wait_and_trigger();
     __shared__ unsigned int s_hist[DIAG ? BIRKHOFF4_HIST_BINS : 1];
@@ -234,7 +236,7 @@ __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void*
         float h[16], T[16];
         load_logits<BF16>(H, idx, h);
         int iters;
-        const unsigned status = lean_forward(h, valid, e_min, tol_i, max_iter, T, iters);
+        const unsigned status = lean_forward(h, valid, lp_range, tol_i, max_iter, T, iters);
         if (valid && status != kLeanFailed) {
             need_robust = 0u;
             store_matrix(P + 16 * idx, T);
@@ -342,7 +344,7 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
     const float tol_i = internal_tol(tol);
     cudaError_t rc = cudaSuccess;
     if (variant >= 3) {
-        const float em = expf(-easy_range());
+        const float em = easy_range();
 #define BK4_LAUNCH_LEAN(T, M)                                                                                     \
     do {                                                                                                          \
         const unsigned g = (unsigned)((B + (T)-1) / (T));                                                         \

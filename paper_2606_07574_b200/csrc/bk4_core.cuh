@@ -366,16 +366,19 @@ BK4_DEV void newton_forward(const V (&H)[16], typename vtraits<V>::mask hard, bo
 }
 
 // -------------------------------------------------------------------------------------------------
-// Lean Newton for well-scaled logits (one matrix per thread, the whole warp in lockstep).
+// Lean Newton (one matrix per thread, the whole warp in lockstep): the path nearly every matrix takes.
 //
 // Same iteration as newton_forward -- eq. (10) for T, eq. (11) for g, the Laplacian form of eq. (12) for the
-// direction, start beta0 = 0 plus one Sinkhorn column step (S1) -- with the guard of DESIGN.md S2 reduced
-// to its test: a step after which the column residual did not fall ends the lean iteration for that matrix,
-// which is then (status kLeanFailed) solved from scratch by newton_forward, whose guard can go back and take
-// Sinkhorn steps.  On logits of small range that happens for a handful of matrices per million, so the common
-// path carries no trial/rollback state, no re-basing and no per-lane stores: a finished lane freezes its v and
-// keeps re-evaluating the same T until the warp is through, and the caller stores all results at once.
+// direction; start beta0 = 0, or the LP dual start for matrices whose largest in-row logit range exceeds
+// `lp_range`, followed by Sinkhorn column steps (S1) -- with the guard of DESIGN.md S2 reduced to its
+// test: a step after which the column residual did not fall ends the lean iteration for that matrix, which is
+// then (status kLeanFailed) solved from scratch by newton_forward, whose guard can go back and take Sinkhorn
+// steps.  Measured on B200: that happens to 0 of 2^20 N(0,1) matrices and to about 1 in 1000 at N(0,30^2).  So
+// the common path carries no trial/rollback state, no re-basing and no per-lane stores: a finished lane freezes
+// its v and keeps re-evaluating the same T until the warp is through, and the caller stores all results at once.
+// A matrix's arithmetic does not depend on the other matrices of its warp.
 //
+//   active    lanes holding a matrix (the others only follow the warp's votes)
 //   returns   kLeanConverged, kLeanStopped (max_iter reached, or the residual stalled at the fp32 floor:
 //             result valid, counted as unconverged) or kLeanFailed (T is not a result)
 constexpr unsigned kLeanConverged = 0u, kLeanStopped = 1u, kLeanFailed = 2u;
@@ -384,31 +387,41 @@ constexpr float kLeanFloorTol = 2e-7f;  // internal tolerances below this are be
 constexpr int kLeanSweeps = 3;       // start-up Sinkhorn column steps
 constexpr int kLeanFree = 2;         // Newton updates taken before the first residual test
 
-//   active    lanes holding a matrix (the others only follow the warp's votes)
-//   e_min     a matrix takes part iff every E_ij = exp(H_ij - max_k H_ik) >= e_min, i.e. its largest in-row logit
-//             range is at most -ln(e_min); the others return kLeanFailed at once (a NaN logit slips through this
-//             test, fails the first residual test and ends up in newton_forward too, which reports it)
-BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float e_min, float tol_i, int max_iter,
+BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float lp_range, float tol_i, int max_iter,
                               float (&T)[16], int& iters) {
     float E[16];
-    // E_ij = exp(H_ij - max_j H_ij): eq. (10) at beta = 0
+    // row maxima (the shift of eq. (10)) and the largest in-row range, which decides the start.
+    // A NaN logit is skipped by fmaxf/fminf: such a matrix fails the first residual test below and ends up in
+    // newton_forward, which reports it; an infinite logit makes the range infinite and is sent there at once.
+    float rmax[4], spread = 0.0f;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const float m = fmaxf(fmaxf(H[4 * i], H[4 * i + 1]), fmaxf(H[4 * i + 2], H[4 * i + 3]));
-        const float t = m * -kLog2e;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) E[4 * i + j] = ex2_approx(fmaf(H[4 * i + j], kLog2e, t));
+        rmax[i] = fmaxf(fmaxf(H[4 * i], H[4 * i + 1]), fmaxf(H[4 * i + 2], H[4 * i + 3]));
+        const float rmin = fminf(fminf(H[4 * i], H[4 * i + 1]), fminf(H[4 * i + 2], H[4 * i + 3]));
+        spread = fmaxf(spread, rmax[i] - rmin);
     }
-    {
-        float lo = fminf(fminf(E[0], E[1]), E[2]);
-#pragma unroll
-        for (int q = 3; q < 15; q += 2) lo = fminf(fminf(lo, E[q]), E[q + 1]);
-        lo = fminf(lo, E[15]);
-        active = active && lo >= e_min;
-    }
+    const bool narrow = active && spread <= lp_range, wide = active && !narrow && spread <= 3.0e38f;
+    active = narrow || wide;  // an infinite (or inf - inf = NaN) range is newton_forward's to report
     iters = 0;
     if (!__any_sync(0xffffffffu, active)) return kLeanFailed;
-    // start-up: kLeanSweeps Sinkhorn column steps from beta = 0 (eq. (6) PAPER.md:108 with the gauge beta_4 = 0;
+    if (__any_sync(0xffffffffu, narrow)) {
+        // E_ij = exp(H_ij - max_j H_ij): eq. (10) at beta0 = 0
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float t = rmax[i] * -kLog2e;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) E[4 * i + j] = ex2_approx(fmaf(H[4 * i + j], kLog2e, t));
+        }
+    }
+    if (__any_sync(0xffffffffu, wide)) {
+        // E at the LP dual start beta0 (log2 units), S1
+        float b0[3], Eg[16];
+        lp_dual_start<float>(H, b0);
+        base_exponentials<float>(H, b0, false, Eg);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) E[q] = wide ? Eg[q] : E[q];
+    }
+    // start-up: kLeanSweeps Sinkhorn column steps from beta0 (eq. (6) PAPER.md:108 with the gauge beta_4 = 0;
     // rows are normalised inside each step, eq. (5)): v_j *= c_4 / c_j.  Each costs a third of a Newton update and
     // cuts the residual about 4x on N(0,1) logits, which is what lets the second Newton update land below 1e-6
     // for 99 % of the matrices instead of 50 % (S1).
@@ -473,12 +486,11 @@ BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float e_min, fl
             g3 = 0.0f;
         }
     };
-    // Newton direction (eq. (12) through the Laplacian form, S7; no ground regularisation: every T_ij of
-    // a matrix that got here is bounded away from 0) and update beta += d  <=>  v *= exp(d)
+    // Newton direction (eq. (12) through the Laplacian form, S7) and update beta += d  <=>  v *= exp(d)
     float d1, d2, d3;
     auto direction = [&]() {
         solve_grounded_laplacian<float>(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), col_dot(T, 0, 3),
-                                        col_dot(T, 1, 3), col_dot(T, 2, 3), g0, g1, g2, 0.0f, d1, d2, d3);
+                                        col_dot(T, 1, 3), col_dot(T, 2, 3), g0, g1, g2, kLamGround, d1, d2, d3);
     };
     // the first kLeanFree updates are taken without looking at the residual: on these inputs no matrix is done
     // before them, and whatever they produce is judged by the tested iterations below
