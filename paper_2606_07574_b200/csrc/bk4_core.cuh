@@ -44,10 +44,12 @@ constexpr float kLamGround = 2.384185791015625e-07f;
 template <class V>
 BK4_DEV void solve_grounded_laplacian(V a, V b, V c, V p, V q, V r, V g1, V g2, V g3, float lam, V& d1, V& d2,
                                       V& d3) {
-    const V l = vsplat(V{}, lam);
-    p = vadd(p, l);
-    q = vadd(q, l);
-    r = vadd(r, l);
+    if (lam != 0.0f) {  // (folds away when the caller has put the regularisation into p, q, r itself)
+        const V l = vsplat(V{}, lam);
+        p = vadd(p, l);
+        q = vadd(q, l);
+        r = vadd(r, l);
+    }
     // eliminate node 1
     const V i1 = vrcp(vadd(vadd(a, b), p));
     const V ai = vmul(a, i1), bi = vmul(b, i1);
@@ -488,9 +490,13 @@ BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float lp_range,
     };
     // Newton direction (eq. (12) through the Laplacian form, S7) and update beta += d  <=>  v *= exp(d)
     float d1, d2, d3;
+    // (the ground regularisation of DESIGN.md S7 rides on the first product of each ground weight's FMA chain)
+    auto ground = [&](int j) {
+        return fmaf(T[12 + j], T[15], fmaf(T[8 + j], T[11], fmaf(T[4 + j], T[7], fmaf(T[j], T[3], kLamGround))));
+    };
     auto direction = [&]() {
-        solve_grounded_laplacian<float>(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), col_dot(T, 0, 3),
-                                        col_dot(T, 1, 3), col_dot(T, 2, 3), g0, g1, g2, kLamGround, d1, d2, d3);
+        solve_grounded_laplacian<float>(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), ground(0), ground(1),
+                                        ground(2), g0, g1, g2, 0.0f, d1, d2, d3);
     };
     // the first kLeanFree updates are taken without looking at the residual: on these inputs no matrix is done
     // before them, and whatever they produce is judged by the tested iterations below
