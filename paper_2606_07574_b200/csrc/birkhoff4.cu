@@ -211,10 +211,10 @@ __global__ void __launch_bounds__(256) forward_kernel(const void* __restrict__ H
 }
 
 // ---------------------------------------------------------------- forward kernel, variants 3 and 4 (default)
-// One matrix per thread.  Every matrix first runs lean_forward in warp lockstep (LP dual start when its largest
-// in-row logit range exceeds lp_range) and the results are stored together; what that leaves (NaN/Inf, or a lean
-// iteration whose residual stopped falling: none in a million N(0,1) matrices, about one in a thousand at
-// N(0,30^2)) runs the guarded newton_forward afterwards, in a branch the warp skips when it has none.
+// One matrix per thread.  Every matrix first runs the lean iteration in warp lockstep (lean_start, lean_iterate:
+// LP dual start when its largest in-row logit range exceeds lp_range) and the results are stored together.  What
+// that leaves (NaN/Inf, a residual that stopped falling: none in a million N(0,1) matrices, about one in a thousand
+// at N(0,30^2)) runs the guarded newton_forward afterwards, in a branch a warp skips when it has none.
 // A matrix's result depends on that matrix alone, not on which matrices share its warp.
 template <bool BF16, bool DIAG, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void* __restrict__ H, float* __restrict__ P,
@@ -228,26 +228,29 @@ __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void*
         if (threadIdx.x == 0) s_unc = 0;
         __syncthreads();
     }
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t b = (int64_t)blockIdx.x * THREADS + threadIdx.x;
     const bool valid = b < B;
     const int64_t idx = valid ? b : B - 1;  // padding lanes shadow the last matrix and store nothing
-    unsigned need_robust = valid ? 1u : 0u;
+    auto finish = [&](const float(&T)[16], int iters, bool converged) {
+        store_matrix(P + 16 * idx, T);
+        if constexpr (DIAG) {
+            if (diag.iters) diag.iters[idx] = iters;
+            atomicAdd(&s_hist[min(iters, BIRKHOFF4_HIST_BINS - 1)], 1u);
+            if (!converged) atomicAdd(&s_unc, 1u);
+        }
+    };
+    bool left = valid;  // this thread's matrix still has to be solved
     {
         float h[16], T[16];
         load_logits<BF16>(H, idx, h);
-        int iters;
-        const unsigned status = lean_forward(h, valid, lp_range, tol_i, max_iter, T, iters);
-        if (valid && status != kLeanFailed) {
-            need_robust = 0u;
-            store_matrix(P + 16 * idx, T);
-            if constexpr (DIAG) {
-                if (diag.iters) diag.iters[idx] = iters;
-                atomicAdd(&s_hist[min(iters, BIRKHOFF4_HIST_BINS - 1)], 1u);
-                if (status != kLeanConverged) atomicAdd(&s_unc, 1u);
-            }
+        LeanState st;
+        if (lean_start(h, valid, lp_range, max_iter, st)) lean_iterate(st, tol_i, max_iter, T);
+        if (valid && st.status != kLeanFailed) {
+            left = false;
+            finish(T, st.it, st.status == kLeanConverged);
         }
     }
-    if (__any_sync(0xffffffffu, need_robust != 0u)) {
+    if (__any_sync(0xffffffffu, left)) {
         float h[16];
         load_logits<BF16>(H, idx, h);  // the lean part has stored only matrices this branch does not touch
         float hmax = h[0], hmin = h[0], poison = 0.0f;
@@ -259,20 +262,15 @@ __global__ void __launch_bounds__(THREADS, MINB) forward_lean_kernel(const void*
         }
         const bool bad = !(poison == 0.0f);
         const bool hard = hmax - hmin > kHardRange;
-        const bool any_hard = __any_sync(0xffffffffu, need_robust != 0u && hard);
+        const bool any_hard = __any_sync(0xffffffffu, left && hard);
         auto reload = [&](float(&Hr)[16]) { load_logits<BF16>(H, idx, Hr); };
         auto emit = [&](int, const float(&T)[16], int iters, bool converged) {
             float out[16];
 #pragma unroll
             for (int q = 0; q < 16; ++q) out[q] = bad ? kNaN : T[q];
-            store_matrix(P + 16 * idx, out);
-            if constexpr (DIAG) {
-                if (diag.iters) diag.iters[idx] = iters;
-                atomicAdd(&s_hist[min(iters, BIRKHOFF4_HIST_BINS - 1)], 1u);
-                if (!converged) atomicAdd(&s_unc, 1u);
-            }
+            finish(out, iters, converged);
         };
-        newton_forward<float, true>(h, bool1(hard), any_hard, bool1(need_robust == 0u), tol_i, max_iter, reload, emit);
+        newton_forward<float, true>(h, bool1(hard), any_hard, bool1(!left), tol_i, max_iter, reload, emit);
     }
     if constexpr (DIAG) {
         __syncthreads();

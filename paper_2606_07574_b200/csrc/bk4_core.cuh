@@ -389,11 +389,66 @@ constexpr float kLeanFloorTol = 2e-7f;  // internal tolerances below this are be
 constexpr int kLeanSweeps = 3;       // start-up Sinkhorn column steps
 constexpr int kLeanFree = 2;         // Newton updates taken before the first residual test
 
-BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float lp_range, float tol_i, int max_iter,
-                              float (&T)[16], int& iters) {
-    float E[16];
+// State of one matrix inside the lean iteration.
+struct LeanState {
+    float E[16];        // exp(beta0_j + H_ij - mu_i), fixed after the start
+    float v0, v1, v2;   // exp(beta_j - beta0_j)
+    float errprev;      // residual of the last update's starting point (kInf before the first tested update)
+    int it;             // updates taken
+    unsigned running;   // 1 while the matrix is being iterated
+    unsigned status;    // kLean* once it is not
+};
+
+// T(beta) of eq. (10) and g_j = c_j - 1 of eq. (11).  REFINE (an evaluation that may be the result): one
+// Newton-Raphson refinement of the SFU reciprocal, so that the rows sum to 1 within rounding, and the residual of
+// all four columns summed as two halves started from -1/2, which keeps every partial sum below 1/2 (S9).
+template <bool REFINE>
+BK4_DEV void lean_eval(const LeanState& s, float (&T)[16], float& g0, float& g1, float& g2, float& g3) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float x0 = s.E[4 * i] * s.v0, x1 = s.E[4 * i + 1] * s.v1, x2 = s.E[4 * i + 2] * s.v2, x3 = s.E[4 * i + 3];
+        const float sum = (x0 + x1) + (x2 + x3);
+        float r = rcp_approx(sum);
+        if constexpr (REFINE) r = fmaf(r, fmaf(-sum, r, 1.0f), r);
+        T[4 * i] = x0 * r;
+        T[4 * i + 1] = x1 * r;
+        T[4 * i + 2] = x2 * r;
+        T[4 * i + 3] = x3 * r;
+    }
+    if constexpr (REFINE) {
+        g0 = ((T[0] - 0.5f) + T[4]) + ((T[8] - 0.5f) + T[12]);
+        g1 = ((T[1] - 0.5f) + T[5]) + ((T[9] - 0.5f) + T[13]);
+        g2 = ((T[2] - 0.5f) + T[6]) + ((T[10] - 0.5f) + T[14]);
+        g3 = ((T[3] - 0.5f) + T[7]) + ((T[11] - 0.5f) + T[15]);
+    } else {
+        g0 = (((T[0] - 1.0f) + T[4]) + T[8]) + T[12];
+        g1 = (((T[1] - 1.0f) + T[5]) + T[9]) + T[13];
+        g2 = (((T[2] - 1.0f) + T[6]) + T[10]) + T[14];
+        g3 = 0.0f;
+    }
+}
+
+// Newton update beta += d <=> v *= exp(d), d from eq. (12) through the Laplacian form (S7); the ground
+// regularisation rides on the first product of each ground weight's FMA chain.
+BK4_DEV void lean_update(LeanState& s, const float (&T)[16], float g0, float g1, float g2, bool apply) {
+    auto ground = [&](int j) {
+        return fmaf(T[12 + j], T[15], fmaf(T[8 + j], T[11], fmaf(T[4 + j], T[7], fmaf(T[j], T[3], kLamGround))));
+    };
+    float d1, d2, d3;
+    solve_grounded_laplacian<float>(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), ground(0), ground(1), ground(2),
+                                    g0, g1, g2, 0.0f, d1, d2, d3);
+    if (apply) {  // a finished lane keeps its v (and so its T)
+        s.v0 *= ex2_approx(d1 * kLog2e);
+        s.v1 *= ex2_approx(d2 * kLog2e);
+        s.v2 *= ex2_approx(d3 * kLog2e);
+    }
+}
+
+// Start: E at beta0 (0, or the LP dual start when the largest in-row range exceeds lp_range), kLeanSweeps Sinkhorn
+// column steps, min(kLeanFree, max_iter) untested Newton updates.  Returns false when the warp has nothing to do.
+BK4_DEV bool lean_start(const float (&H)[16], bool active, float lp_range, int max_iter, LeanState& s) {
     // row maxima (the shift of eq. (10)) and the largest in-row range, which decides the start.
-    // A NaN logit is skipped by fmaxf/fminf: such a matrix fails the first residual test below and ends up in
+    // A NaN logit is skipped by fmaxf/fminf: such a matrix fails the first residual test and ends up in
     // newton_forward, which reports it; an infinite logit makes the range infinite and is sent there at once.
     float rmax[4], spread = 0.0f;
 #pragma unroll
@@ -404,15 +459,18 @@ BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float lp_range,
     }
     const bool narrow = active && spread <= lp_range, wide = active && !narrow && spread <= 3.0e38f;
     active = narrow || wide;  // an infinite (or inf - inf = NaN) range is newton_forward's to report
-    iters = 0;
-    if (!__any_sync(0xffffffffu, active)) return kLeanFailed;
+    s.running = active ? 1u : 0u;
+    s.status = kLeanFailed;
+    s.errprev = kInf;
+    s.it = 0;
+    if (!__any_sync(0xffffffffu, active)) return false;
     if (__any_sync(0xffffffffu, narrow)) {
         // E_ij = exp(H_ij - max_j H_ij): eq. (10) at beta0 = 0
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const float t = rmax[i] * -kLog2e;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) E[4 * i + j] = ex2_approx(fmaf(H[4 * i + j], kLog2e, t));
+            for (int j = 0; j < 4; ++j) s.E[4 * i + j] = ex2_approx(fmaf(H[4 * i + j], kLog2e, t));
         }
     }
     if (__any_sync(0xffffffffu, wide)) {
@@ -421,120 +479,66 @@ BK4_DEV unsigned lean_forward(const float (&H)[16], bool active, float lp_range,
         lp_dual_start<float>(H, b0);
         base_exponentials<float>(H, b0, false, Eg);
 #pragma unroll
-        for (int q = 0; q < 16; ++q) E[q] = wide ? Eg[q] : E[q];
+        for (int q = 0; q < 16; ++q) s.E[q] = wide ? Eg[q] : s.E[q];
     }
-    // start-up: kLeanSweeps Sinkhorn column steps from beta0 (eq. (6) PAPER.md:108 with the gauge beta_4 = 0;
-    // rows are normalised inside each step, eq. (5)): v_j *= c_4 / c_j.  Each costs a third of a Newton update and
-    // cuts the residual about 4x on N(0,1) logits, which is what lets the second Newton update land below 1e-6
-    // for 99 % of the matrices instead of 50 % (S1).
-    float v0, v1, v2;
-    {
+    // kLeanSweeps Sinkhorn column steps from beta0 (eq. (6) PAPER.md:108 with the gauge beta_4 = 0; rows are
+    // normalised inside each step, eq. (5)): v_j *= c_4 / c_j.  Each costs a third of a Newton update and cuts the
+    // residual about 4x on N(0,1) logits, which is what lets the second Newton update land below 1e-6 for 99 % of
+    // the matrices instead of 50 % (S1).
+    s.v0 = s.v1 = s.v2 = 1.0f;
+#pragma unroll
+    for (int k = 0; k < kLeanSweeps; ++k) {
         float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            const float r = rcp_approx((E[4 * i] + E[4 * i + 1]) + (E[4 * i + 2] + E[4 * i + 3]));
-            c0 = fmaf(E[4 * i], r, c0);
-            c1 = fmaf(E[4 * i + 1], r, c1);
-            c2 = fmaf(E[4 * i + 2], r, c2);
-            c3 = fmaf(E[4 * i + 3], r, c3);
-        }
-        v0 = c3 * rcp_approx(c0);
-        v1 = c3 * rcp_approx(c1);
-        v2 = c3 * rcp_approx(c2);
-    }
-#pragma unroll
-    for (int k = 1; k < kLeanSweeps; ++k) {
-        float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const float x0 = E[4 * i] * v0, x1 = E[4 * i + 1] * v1, x2 = E[4 * i + 2] * v2, x3 = E[4 * i + 3];
+            const float x0 = k ? s.E[4 * i] * s.v0 : s.E[4 * i], x1 = k ? s.E[4 * i + 1] * s.v1 : s.E[4 * i + 1],
+                        x2 = k ? s.E[4 * i + 2] * s.v2 : s.E[4 * i + 2], x3 = s.E[4 * i + 3];
             const float r = rcp_approx((x0 + x1) + (x2 + x3));
             c0 = fmaf(x0, r, c0);
             c1 = fmaf(x1, r, c1);
             c2 = fmaf(x2, r, c2);
             c3 = fmaf(x3, r, c3);
         }
-        v0 *= c3 * rcp_approx(c0);
-        v1 *= c3 * rcp_approx(c1);
-        v2 *= c3 * rcp_approx(c2);
+        const float f0 = c3 * rcp_approx(c0), f1 = c3 * rcp_approx(c1), f2 = c3 * rcp_approx(c2);
+        s.v0 = k ? s.v0 * f0 : f0;
+        s.v1 = k ? s.v1 * f1 : f1;
+        s.v2 = k ? s.v2 * f2 : f2;
     }
-    // T(beta) of eq. (10) and g_j = c_j - 1 of eq. (11), accumulated from -1 so that the partial sums stay below 1
-    // in magnitude (S9).  REFINE: one Newton-Raphson refinement of the SFU reciprocal, so that the rows
-    // of a T that may be the result sum to 1 within rounding.
-    float g0, g1, g2, g3;
-    auto eval = [&](auto refine) {
-        constexpr bool kRefine = decltype(refine)::value;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const float x0 = E[4 * i] * v0, x1 = E[4 * i + 1] * v1, x2 = E[4 * i + 2] * v2, x3 = E[4 * i + 3];
-            const float s = (x0 + x1) + (x2 + x3);
-            float r = rcp_approx(s);
-            if constexpr (kRefine) r = fmaf(r, fmaf(-s, r, 1.0f), r);
-            T[4 * i] = x0 * r;
-            T[4 * i + 1] = x1 * r;
-            T[4 * i + 2] = x2 * r;
-            T[4 * i + 3] = x3 * r;
-        }
-        if constexpr (kRefine) {
-            // tested residual: two half sums, each started from -1/2, keep every partial sum below 1/2
-            g0 = ((T[0] - 0.5f) + T[4]) + ((T[8] - 0.5f) + T[12]);
-            g1 = ((T[1] - 0.5f) + T[5]) + ((T[9] - 0.5f) + T[13]);
-            g2 = ((T[2] - 0.5f) + T[6]) + ((T[10] - 0.5f) + T[14]);
-            g3 = ((T[3] - 0.5f) + T[7]) + ((T[11] - 0.5f) + T[15]);
-        } else {
-            g0 = (((T[0] - 1.0f) + T[4]) + T[8]) + T[12];
-            g1 = (((T[1] - 1.0f) + T[5]) + T[9]) + T[13];
-            g2 = (((T[2] - 1.0f) + T[6]) + T[10]) + T[14];
-            g3 = 0.0f;
-        }
-    };
-    // Newton direction (eq. (12) through the Laplacian form, S7) and update beta += d  <=>  v *= exp(d)
-    float d1, d2, d3;
-    // (the ground regularisation of DESIGN.md S7 rides on the first product of each ground weight's FMA chain)
-    auto ground = [&](int j) {
-        return fmaf(T[12 + j], T[15], fmaf(T[8 + j], T[11], fmaf(T[4 + j], T[7], fmaf(T[j], T[3], kLamGround))));
-    };
-    auto direction = [&]() {
-        solve_grounded_laplacian<float>(col_dot(T, 0, 1), col_dot(T, 0, 2), col_dot(T, 1, 2), ground(0), ground(1),
-                                        ground(2), g0, g1, g2, 0.0f, d1, d2, d3);
-    };
-    // the first kLeanFree updates are taken without looking at the residual: on these inputs no matrix is done
-    // before them, and whatever they produce is judged by the tested iterations below
+    // the first kLeanFree updates are taken without looking at the residual: on well-scaled inputs no matrix is
+    // done before them, and whatever they produce is judged by the tested iterations of lean_iterate
     const int n_free = max_iter < kLeanFree ? max_iter : kLeanFree;
     for (int k = 0; k < n_free; ++k) {
-        eval(std::false_type{});
-        direction();
-        v0 *= ex2_approx(d1 * kLog2e);
-        v1 *= ex2_approx(d2 * kLog2e);
-        v2 *= ex2_approx(d3 * kLog2e);
+        float T[16], g0, g1, g2, g3;
+        lean_eval<false>(s, T, g0, g1, g2, g3);
+        lean_update(s, T, g0, g1, g2, true);
     }
-    float errprev = kInf;
-    unsigned running = active ? 1u : 0u, status = kLeanFailed;
-    int it = n_free;
+    s.it = n_free;
+    return true;
+}
+
+// Tested iterations in warp lockstep: evaluate, stop test, Newton update, until no lane is running.
+// T holds the last evaluation of every lane: the result of the lanes whose status is not kLeanFailed.
+BK4_DEV void lean_iterate(LeanState& s, float tol_i, int max_iter, float (&T)[16]) {
     for (;;) {
-        eval(std::true_type{});
+        float g0, g1, g2, g3;
+        lean_eval<true>(s, T, g0, g1, g2, g3);
         const float err = (fabsf(g0) + fabsf(g1)) + (fabsf(g2) + fabsf(g3));
         const bool conv = err <= tol_i;  // false for NaN: a NaN ends up in newton_forward
-        const bool improved = err < errprev;
-        if (running && (conv || !improved || it >= max_iter)) {
-            running = 0u;
+        const bool improved = err < s.errprev;
+        if (s.running && (conv || !improved || s.it >= max_iter)) {
+            s.running = 0u;
             // a residual that no longer falls: the fp32 floor if the caller asked for less than fp32 can give,
             // otherwise newton_forward's Sinkhorn steps may still get below tol
-            status = conv ? kLeanConverged
-                          : (improved || (errprev < kLeanFloor && tol_i < kLeanFloorTol)) ? kLeanStopped : kLeanFailed;
+            s.status = conv ? kLeanConverged
+                            : (improved || (s.errprev < kLeanFloor && tol_i < kLeanFloorTol)) ? kLeanStopped : kLeanFailed;
         }
-        if (!__any_sync(0xffffffffu, running != 0u)) break;
-        direction();
-        if (running) {  // a finished lane keeps its v (and so its T)
-            v0 *= ex2_approx(d1 * kLog2e);
-            v1 *= ex2_approx(d2 * kLog2e);
-            v2 *= ex2_approx(d3 * kLog2e);
-            errprev = err;
-            ++it;
+        if (!__any_sync(0xffffffffu, s.running != 0u)) break;
+        lean_update(s, T, g0, g1, g2, s.running != 0u);
+        if (s.running) {
+            s.errprev = err;
+            ++s.it;
         }
     }
-    iters = it;
-    return status;
 }
 
 // -------------------------------------------------------------------------------------------------
