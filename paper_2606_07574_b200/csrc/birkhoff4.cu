@@ -85,7 +85,7 @@ BK4_DEV void load_logits(const void* H, int64_t b, float (&m)[16]) {
 // logit range (max - min over the 16 entries) above which a matrix takes the LP dual start (S1):
 // N(0,1) logits stay below it, N(0,2^2) and larger mostly exceed it.
 constexpr float kHardRange = 8.0f;
-// largest in-row logit range up to which lean_forward starts from beta = 0 (above: LP dual start); chosen by
+// largest in-row logit range up to which lean_start starts from beta = 0 (above: LP dual start); chosen by
 // measurement, DESIGN.md
 constexpr float kEasyRange = 12.0f;
 

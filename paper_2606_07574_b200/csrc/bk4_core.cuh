@@ -252,7 +252,7 @@ BK4_DEV void lp_dual_start(const V (&H)[16], V (&b0)[3]) {
 // `any_hard` must be uniform over the threads that execute together (it only selects the cheaper start-up
 // code when no matrix needs the LP start).  Reload(H) re-reads the logits (used when the base point moves);
 // Emit(half, T, iters, converged) receives the result of one matrix as soon as it is final.
-// `skip` marks matrices this call must leave alone (already finished by lean_forward, or padding): they start out
+// `skip` marks matrices this call must leave alone (already finished by lean_iterate, or padding): they start out
 // `done`, nothing is emitted for them and their arithmetic is ignored.
 // LANE_INDEPENDENT: a matrix's arithmetic does not depend on which other matrices share its warp (the cheaper
 // start-up code for warps without a `hard` matrix rounds differently), at the cost of a few instructions.
