@@ -283,11 +283,11 @@ def run_ours(args, wl):
     max_err, mean_err = float(err.max()), float(err.mean())
     hist = torch.zeros(64, dtype=torch.int64, device="cuda")
     unc = torch.zeros(1, dtype=torch.int64, device="cuda")
-    if not bf16:
-        bk.birkhoff4_forward_ex(sets[0]["H"], sets[0]["P"], TOL, max_iter, hist=hist, n_unconverged=unc)
+    (bk.birkhoff4_forward_bf16_ex if bf16 else bk.birkhoff4_forward_ex)(sets[0]["H"], sets[0]["P"], TOL, max_iter,
+                                                                        hist=hist, n_unconverged=unc)
     h = hist.cpu().numpy()
-    mean_updates = float((h * np.arange(64)).sum() / max(h.sum(), 1)) if not bf16 else None
-    update_hist = {str(k): round(float(h[k]) / max(h.sum(), 1), 6) for k in range(64) if h[k]} if not bf16 else None
+    mean_updates = float((h * np.arange(64)).sum() / max(h.sum(), 1))
+    update_hist = {str(k): round(float(h[k]) / max(h.sum(), 1), 6) for k in range(64) if h[k]}
     del P64, err
 
     # ---- Sinkhorn-20 baseline kernel of the same library (context: PAPER.md:32, 319), fp32 workloads only

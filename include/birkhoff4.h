@@ -81,6 +81,10 @@ int birkhoff4_forward_ex(const float* H, float* P, int64_t B, float tol, int max
 /* Forward for logits stored as bf16 bit patterns (uint16 [B][4][4], 32 B per matrix); P is fp32. */
 int birkhoff4_forward_bf16(const uint16_t* H, float* P, int64_t B, float tol, int max_iter,
                            birkhoff4_stream_t stream);
+/* The same with the diagnostics of birkhoff4_forward_ex (each nullable). */
+int birkhoff4_forward_bf16_ex(const uint16_t* H, float* P, int64_t B, float tol, int max_iter, int32_t* iters,
+                              unsigned long long* hist, unsigned long long* n_unconverged,
+                              birkhoff4_stream_t stream);
 
 /*
  * Backward (section 4.2).  P: the forward output; dP = dL/dP; dH = dL/dH, all

@@ -32,6 +32,7 @@ def lib():
         L.birkhoff4_forward.argtypes = [vp, vp, i64, f32, ci, vp]
         L.birkhoff4_forward_ex.argtypes = [vp, vp, i64, f32, ci, vp, vp, vp, vp]
         L.birkhoff4_forward_bf16.argtypes = [vp, vp, i64, f32, ci, vp]
+        L.birkhoff4_forward_bf16_ex.argtypes = [vp, vp, i64, f32, ci, vp, vp, vp, vp]
         L.birkhoff4_backward.argtypes = [vp, vp, vp, i64, vp]
         L.birkhoff4_sinkhorn.argtypes = [vp, vp, i64, ci, vp]
         L.birkhoff4_forward_host.argtypes = [vp, vp, i64, f32, ci]
@@ -43,7 +44,7 @@ def lib():
         L.birkhoff4_strerror.argtypes = [ci]
         L.birkhoff4_strerror.restype = ctypes.c_char_p
         L.birkhoff4_version.argtypes = []
-        for name in ("forward", "forward_ex", "forward_bf16", "backward", "sinkhorn", "forward_host",
+        for name in ("forward", "forward_ex", "forward_bf16", "forward_bf16_ex", "backward", "sinkhorn", "forward_host",
                      "backward_host", "forward_backward_host", "set_variant", "version"):
             getattr(L, "birkhoff4_" + name).restype = ci
         _LIB = L
@@ -85,11 +86,7 @@ def birkhoff4_forward(H, P=None, tol=1e-6, max_iter=20, stream=None):
     return P
 
 
-def birkhoff4_forward_ex(H, P=None, tol=1e-6, max_iter=20, iters=None, hist=None, n_unconverged=None, stream=None):
-    """forward + diagnostics; iters int32[B], hist int64[64] (accumulated), n_unconverged int64[1] (accumulated)"""
-    H = _dev(H, torch.float32, "H")
-    P = torch.empty_like(H) if P is None else _dev(P, torch.float32, "P")
-    B = H.numel() // 16
+def _diag_check(B, iters, hist, n_unconverged):
     if iters is not None and (iters.dtype != torch.int32 or iters.numel() != B or not iters.is_cuda):
         raise Birkhoff4Error("iters must be a CUDA int32 tensor of [B]")
     if hist is not None and (hist.dtype != torch.int64 or hist.numel() != HIST_BINS or not hist.is_cuda):
@@ -97,6 +94,14 @@ def birkhoff4_forward_ex(H, P=None, tol=1e-6, max_iter=20, iters=None, hist=None
     if n_unconverged is not None and (n_unconverged.dtype != torch.int64 or n_unconverged.numel() != 1
                                       or not n_unconverged.is_cuda):
         raise Birkhoff4Error("n_unconverged must be a CUDA int64 tensor of [1]")
+
+
+def birkhoff4_forward_ex(H, P=None, tol=1e-6, max_iter=20, iters=None, hist=None, n_unconverged=None, stream=None):
+    """forward + diagnostics; iters int32[B], hist int64[64] (accumulated), n_unconverged int64[1] (accumulated)"""
+    H = _dev(H, torch.float32, "H")
+    P = torch.empty_like(H) if P is None else _dev(P, torch.float32, "P")
+    B = H.numel() // 16
+    _diag_check(B, iters, hist, n_unconverged)
     _check(lib().birkhoff4_forward_ex(_ptr(H), _ptr(P), B, tol, max_iter, _ptr(iters), _ptr(hist),
                                       _ptr(n_unconverged), _stream(stream)))
     return P
@@ -107,6 +112,17 @@ def birkhoff4_forward_bf16(H, P=None, tol=1e-6, max_iter=20, stream=None):
     H = _dev(H, torch.bfloat16, "H")
     P = torch.empty(H.shape, dtype=torch.float32, device=H.device) if P is None else _dev(P, torch.float32, "P")
     _check(lib().birkhoff4_forward_bf16(_ptr(H), _ptr(P), H.numel() // 16, tol, max_iter, _stream(stream)))
+    return P
+
+
+def birkhoff4_forward_bf16_ex(H, P=None, tol=1e-6, max_iter=20, iters=None, hist=None, n_unconverged=None, stream=None):
+    """bf16-logit forward + the diagnostics of birkhoff4_forward_ex"""
+    H = _dev(H, torch.bfloat16, "H")
+    P = torch.empty(H.shape, dtype=torch.float32, device=H.device) if P is None else _dev(P, torch.float32, "P")
+    B = H.numel() // 16
+    _diag_check(B, iters, hist, n_unconverged)
+    _check(lib().birkhoff4_forward_bf16_ex(_ptr(H), _ptr(P), B, tol, max_iter, _ptr(iters), _ptr(hist),
+                                           _ptr(n_unconverged), _stream(stream)))
     return P
 
 

@@ -463,6 +463,11 @@ int birkhoff4_forward_bf16(const uint16_t* H, float* P, int64_t B, float tol, in
     return launch_forward<true>(H, P, B, tol, max_iter, FwdDiag{nullptr, nullptr, nullptr}, (cudaStream_t)stream);
 }
 
+int birkhoff4_forward_bf16_ex(const uint16_t* H, float* P, int64_t B, float tol, int max_iter, int32_t* iters,
+                              unsigned long long* hist, unsigned long long* n_unconverged, birkhoff4_stream_t stream) {
+    return launch_forward<true>(H, P, B, tol, max_iter, FwdDiag{iters, hist, n_unconverged}, (cudaStream_t)stream);
+}
+
 int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, birkhoff4_stream_t stream) {
     if (B < 0) return BIRKHOFF4_EINVAL;
     if (B == 0) return BIRKHOFF4_OK;

@@ -207,6 +207,20 @@ def test_config4_full_size(oracle):
     print("config4", _full_size(oracle, c["H_f32"], c["G"], P, 4096, 3e-6, 4))
 
 
+def test_bf16_diagnostics_match_fp32_path():
+    """bf16 logits widen exactly, so the bf16 entry points must equal the fp32 ones on the widened values"""
+    c = inputs.make(4, B=50001)
+    Hb = torch.from_numpy(c["H"].view(np.int16)).cuda().view(torch.bfloat16)
+    Hf = dev(c["H_f32"])
+    ib, i32 = (torch.zeros(50001, dtype=torch.int32, device="cuda") for _ in range(2))
+    hb, h32 = (torch.zeros(64, dtype=torch.int64, device="cuda") for _ in range(2))
+    Pb = bk.birkhoff4_forward_bf16_ex(Hb, iters=ib, hist=hb)
+    P32 = bk.birkhoff4_forward_ex(Hf, iters=i32, hist=h32)
+    assert torch.equal(Pb, P32) and torch.equal(ib, i32) and torch.equal(hb, h32)
+    assert torch.equal(bk.birkhoff4_forward_bf16(Hb), Pb)
+    assert int(hb.sum()) == 50001
+
+
 def test_config5_full_size(oracle):
     c = inputs.make(5)
     P = bk.birkhoff4_forward(dev(c["H"]), max_iter=32)
