@@ -529,6 +529,25 @@ def test_sinkhorn20_table2_statistics(oracle):
     assert abs(err.mean() - mean) < 0.05 * mean and abs(np.median(err) - med) < 0.05 * med
 
 
+def test_marginal_error_not_worse_than_the_papers_solver(oracle):
+    """Tables 1-2 (tests/golden/paper_tables_newton_err.txt): same distributions, N = 10^4, tol 1e-6, max_iter 20"""
+    import os
+    rows = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_tables_newton_err.txt")) as f:
+        for line in f:
+            if not line.startswith("#") and line.strip():
+                k = line.split()
+                u = float(k[1])
+                rows[k[0]] = dict(mean=float(k[2]) * u, median=float(k[4]) * u, max=float(k[5]) * u)
+    draws = {"N(0,1)": inputs.normal(10000, 1.0, config=81)[0], "Unif(-1,1)": inputs.uniform(10000, 1.0, config=82)[0],
+             "N(0,10^2)": inputs.normal(10000, 10.0, config=83)[0], "Unif(-10,10)": inputs.uniform(10000, 10.0, config=84)[0]}
+    for name, H in draws.items():
+        err = oracle.marginal_err(gpu_forward(H, tol=1e-6, max_iter=20))
+        print(name, "Err mean %.3e median %.3e max %.3e   paper %s" % (err.mean(), np.median(err), err.max(), rows[name]))
+        assert err.mean() <= rows[name]["mean"] and err.max() <= rows[name]["max"]
+        assert err.max() <= 3e-6                                                 # and converged everywhere, unlike Table 2
+
+
 # ---------------------------------------------------------------------------------------------------
 # host-buffer entry points (the end-to-end path bench.py times): same bits as the device-pointer calls
 @pytest.mark.parametrize("B", [1, 1000, (1 << 18) + 17, (1 << 19) * 3 + 5])
