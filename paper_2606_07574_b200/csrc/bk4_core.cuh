@@ -388,6 +388,7 @@ constexpr float kLeanFloor = 1e-5f;  // a residual that stalls below this is the
 constexpr float kLeanFloorTol = 2e-7f;  // internal tolerances below this are below the fp32 floor of the residual
 constexpr int kLeanSweeps = 3;       // start-up Sinkhorn column steps
 constexpr int kLeanFree = 2;         // Newton updates taken before the first residual test
+constexpr float kBalanceFloor = 3e-6f;  // floor of the flows in the balancing step after the LP start
 
 // State of one matrix inside the lean iteration.
 struct LeanState {
@@ -486,8 +487,10 @@ BK4_DEV bool lean_start(const float (&H)[16], bool active, float lp_range, int m
     // residual about 4x on N(0,1) logits, which is what lets the second Newton update land below 1e-6 for 99 % of
     // the matrices instead of 50 % (S1).
     s.v0 = s.v1 = s.v2 = 1.0f;
+    const bool any_narrow = __any_sync(0xffffffffu, narrow), any_wide = __any_sync(0xffffffffu, wide);
 #pragma unroll
     for (int k = 0; k < kLeanSweeps; ++k) {
+        if (k > 0 && !any_narrow) break;  // matrices with the LP start take the first step only (see below)
         float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -500,9 +503,48 @@ BK4_DEV bool lean_start(const float (&H)[16], bool active, float lp_range, int m
             c3 = fmaf(x3, r, c3);
         }
         const float f0 = c3 * rcp_approx(c0), f1 = c3 * rcp_approx(c1), f2 = c3 * rcp_approx(c2);
-        s.v0 = k ? s.v0 * f0 : f0;
-        s.v1 = k ? s.v1 * f1 : f1;
-        s.v2 = k ? s.v2 * f2 : f2;
+        if (k == 0) {
+            s.v0 = f0, s.v1 = f1, s.v2 = f2;
+        } else if (narrow) {
+            s.v0 *= f0, s.v1 *= f1, s.v2 *= f2;
+        }
+    }
+    // Matrices with the LP start: their T is a permutation matrix plus small entries, where column steps barely
+    // move (Sinkhorn's slow regime) and Newton's updates are of unit size, so that the residual
+    // falls by a factor e per update only.  What has to happen is that the small entries get balanced: column
+    // j's inflow in_j = c_j - max_i T_ij against the outflow out_j = 1 - max_i T_ij of the row holding its
+    // dominant entry.  One balancing step beta_j += (1/2) log(out_j / in_j) (Osborne's matrix-balancing update,
+    // gauge beta_4 = 0) jumps there; flows are floored at kBalanceFloor, above the fp32 noise of 1 - max.  It is
+    // a start-up step like the column steps: whatever it produces is judged by the tested iterations.  Measured
+    // (S1): the mean over warps of the largest update count falls from 6.8 to 4.5 at N(0,100^2).
+    if (any_wide) {
+        float c[4] = {0.0f, 0.0f, 0.0f, 0.0f}, m[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float x0 = s.E[4 * i] * s.v0, x1 = s.E[4 * i + 1] * s.v1, x2 = s.E[4 * i + 2] * s.v2, x3 = s.E[4 * i + 3];
+            const float r = rcp_approx((x0 + x1) + (x2 + x3));
+            const float t[4] = {x0 * r, x1 * r, x2 * r, x3 * r};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                c[j] += t[j];
+                m[j] = fmaxf(m[j], t[j]);
+            }
+        }
+        float in[4], out[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            in[j] = fmaxf(c[j] - m[j], 0.0f) + kBalanceFloor;
+            out[j] = fmaxf(1.0f - m[j], 0.0f) + kBalanceFloor;
+        }
+        // v_j *= sqrt((out_j / in_j) / (out_4 / in_4))
+        const float num = in[3], den = out[3];
+        const float q0 = (out[0] * num) * rcp_approx(in[0] * den), q1 = (out[1] * num) * rcp_approx(in[1] * den),
+                    q2 = (out[2] * num) * rcp_approx(in[2] * den);
+        if (wide) {
+            s.v0 *= sqrt_approx(q0);
+            s.v1 *= sqrt_approx(q1);
+            s.v2 *= sqrt_approx(q2);
+        }
     }
     // the first kLeanFree updates are taken without looking at the residual: on well-scaled inputs no matrix is
     // done before them, and whatever they produce is judged by the tested iterations of lean_iterate
