@@ -344,6 +344,17 @@ def run_ours(args, wl):
     }
     for name, k in kernels.items():
         k.update(peak=peak, unit="GB/s", frac=k["achieved"] / peak, traffic=ncu_traffic(name, B))
+    # the forward's second roofline: plain FP32 arithmetic.  Algorithmic work = 150 FP32 thread
+    # instructions per evaluation of T, g, Hessian and solve (eqs. (10)-(12)) x (mean updates + 1 final evaluation
+    # + 1 for the start-up steps); peak = 128 FP32 lanes per clock per SM at the maximum SM clock.
+    props = torch.cuda.get_device_properties(local)
+    sm_mhz = clocks.max_mhz or 1965
+    alu_peak = 128.0 * props.multi_processor_count * sm_mhz * 1e6 / 1e12
+    alu_work = 150.0 * (mean_updates + 2.0)
+    alu_ach = B * alu_work / (f_ms * 1e-3) / 1e12
+    kernels["forward_lean_kernel"]["alu"] = {
+        "bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T FP32 instr/s", "frac": alu_ach / alu_peak,
+        "fp32_instr_per_matrix": alu_work}
     dom = "forward_lean_kernel" if f_ms >= b_ms else "backward_kernel"
     roofline = dict(kernels[dom], kernel=dom, peak_source=peak_src)
     out = {
