@@ -468,6 +468,34 @@ def test_non_default_stream():
     assert torch.equal(P, ref) and torch.equal(dH, ref_d)
 
 
+def test_legacy_default_stream_and_stream_order():
+    """stream 0 through the raw C ABI, and a dependent chain on one stream (forward -> backward -> forward in place):
+    programmatic dependent launch must not let a kernel read what its predecessor has not written yet"""
+    import ctypes
+    H, G = inputs.normal((1 << 18) + 3, 2.0, config=70)
+    Hd, Gd = dev(H), dev(G)
+    ref = bk.birkhoff4_forward(Hd)
+    ref_d = bk.birkhoff4_backward(ref, Gd)
+    ref_2 = bk.birkhoff4_forward(ref_d)
+    torch.cuda.synchronize()
+    L, B = bk.lib(), Hd.shape[0]
+    P, dH = torch.empty_like(Hd), torch.empty_like(Hd)
+    torch.cuda.synchronize()
+    null = ctypes.c_void_p(0)
+    assert L.birkhoff4_forward(ctypes.c_void_p(Hd.data_ptr()), ctypes.c_void_p(P.data_ptr()), B, 1e-6, 20, null) == 0
+    assert L.birkhoff4_backward(ctypes.c_void_p(P.data_ptr()), ctypes.c_void_p(Gd.data_ptr()),
+                                ctypes.c_void_p(dH.data_ptr()), B, null) == 0
+    torch.cuda.synchronize()
+    assert torch.equal(P, ref) and torch.equal(dH, ref_d)
+    for _ in range(20):                                                          # back-to-back dependent launches
+        P.zero_(), dH.zero_()
+        bk.birkhoff4_forward(Hd, P)
+        bk.birkhoff4_backward(P, Gd, dH)
+        bk.birkhoff4_forward(dH, dH)
+        torch.cuda.synchronize()
+        assert torch.equal(P, ref) and torch.equal(dH, ref_2)
+
+
 # ---------------------------------------------------------------------------------------------------
 # backward on its own: fed the oracle's P (rounded to fp32), including near-permutation P where the
 # paper's Delta is singular (DESIGN.md S7)
