@@ -445,8 +445,9 @@ BK4_DEV void lean_update(LeanState& s, const float (&T)[16], float g0, float g1,
     }
 }
 
-// Start: E at beta0 (0, or the LP dual start when the largest in-row range exceeds lp_range), kLeanSweeps Sinkhorn
-// column steps, min(kLeanFree, max_iter) untested Newton updates.  Returns false when the warp has nothing to do.
+// Start: E at beta0 (0, or the LP dual start when the largest in-row range exceeds lp_range), then kLeanSweeps
+// Sinkhorn column steps (beta0 = 0) or one balancing step (LP start), then min(kLeanFree, max_iter) untested Newton
+// updates.  Returns false when the warp has nothing to do.
 BK4_DEV bool lean_start(const float (&H)[16], bool active, float lp_range, int max_iter, LeanState& s) {
     // row maxima (the shift of eq. (10)) and the largest in-row range, which decides the start.
     // A NaN logit is skipped by fmaxf/fminf: such a matrix fails the first residual test and ends up in
@@ -490,7 +491,7 @@ BK4_DEV bool lean_start(const float (&H)[16], bool active, float lp_range, int m
     const bool any_narrow = __any_sync(0xffffffffu, narrow), any_wide = __any_sync(0xffffffffu, wide);
 #pragma unroll
     for (int k = 0; k < kLeanSweeps; ++k) {
-        if (k > 0 && !any_narrow) break;  // matrices with the LP start take the first step only (see below)
+        if (!any_narrow) break;  // matrices with the LP start take the balancing step below instead
         float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -503,11 +504,7 @@ BK4_DEV bool lean_start(const float (&H)[16], bool active, float lp_range, int m
             c3 = fmaf(x3, r, c3);
         }
         const float f0 = c3 * rcp_approx(c0), f1 = c3 * rcp_approx(c1), f2 = c3 * rcp_approx(c2);
-        if (k == 0) {
-            s.v0 = f0, s.v1 = f1, s.v2 = f2;
-        } else if (narrow) {
-            s.v0 *= f0, s.v1 *= f1, s.v2 *= f2;
-        }
+        if (narrow) s.v0 *= f0, s.v1 *= f1, s.v2 *= f2;
     }
     // Matrices with the LP start: their T is a permutation matrix plus small entries, where column steps barely
     // move (Sinkhorn's slow regime) and Newton's updates are of unit size, so that the residual
