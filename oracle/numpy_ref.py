@@ -44,7 +44,10 @@ def kkt_matrix(P):
 
 
 def backward_pinv(P, G, rcond=1e-13):
-    """dH_ij = P_ij (G_ij - v_i - w_j), [v;w] = K^+ [(GoP)1; (GoP)^T 1]   (PAPER.md:527-563 ungauged)."""
+    """dH_ij = P_ij (G_ij - v_i - w_j), [v;w] = K^+ [(GoP)1; (GoP)^T 1]   (PAPER.md:527-563 ungauged).
+    Valid for well-scaled logits only (|H| of a few units): LAPACK's eigen-solver loses the small eigenvalues of K
+    that the C oracle's Jacobi sweep keeps, and at N(0,10^2) and above this write-up is off by up to 1e-3.  The
+    tests use it at s <= 3; at s >= 10 the value pin is an 80-digit solve (tests/test_oracle_backward.py)."""
     P = np.asarray(P, np.float64).reshape(-1, 4, 4)
     G = np.asarray(G, np.float64).reshape(-1, 4, 4)
     Gam = G * P

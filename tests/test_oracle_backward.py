@@ -27,6 +27,47 @@ def test_backward_matches_finite_differences(oracle, s):
     assert np.abs(dH - numpy_ref.backward_pinv(P, G)).max() < 1e-13
 
 
+# ---- P10b: value pin at LARGE scale: the gauge-fixed 7x7 system (PAPER.md:543-563 with w_4 = 0) solved in 80-digit
+# arithmetic.  The library pinv of numpy_ref.backward_pinv loses the small eigenvalues there (off by up to 1e-3 at
+# s >= 10) and is NOT the cross-check at these scales; this is.
+def _backward_exact_mp(P, G):
+    import mpmath as mp
+    with mp.workdps(80):
+        Pm = [[mp.mpf(float(P[i, j])) for j in range(4)] for i in range(4)]
+        Gm = [[mp.mpf(float(G[i, j])) for j in range(4)] for i in range(4)]
+        K, rhs = mp.zeros(7, 7), mp.zeros(7, 1)
+        for i in range(4):
+            K[i, i] = sum(Pm[i])                                           # diag(r)
+            rhs[i] = sum(Gm[i][j] * Pm[i][j] for j in range(4))            # mu_r
+            for j in range(3):
+                K[i, 4 + j] = K[4 + j, i] = Pm[i][j]
+        for j in range(3):
+            K[4 + j, 4 + j] = sum(Pm[i][j] for i in range(4))              # diag(c), last column dropped (gauge)
+            rhs[4 + j] = sum(Gm[i][j] * Pm[i][j] for i in range(4))        # mu_c
+        y = mp.lu_solve(K, rhs)
+        v, w = [y[i] for i in range(4)], [y[4], y[5], y[6], mp.mpf(0)]
+        return np.array([[float(Pm[i][j] * (Gm[i][j] - v[i] - w[j])) for j in range(4)] for i in range(4)])
+
+
+@pytest.mark.parametrize("s", [10.0, 30.0, 100.0])
+def test_backward_large_scale_against_80_digit_solve(oracle, s):
+    H, G = inputs.normal(64, s, config=51, sub=7)
+    P = oracle.forward(H)
+    dH = oracle.backward(P, G)
+    checked, worst = 0, 0.0
+    for b in range(64):
+        if P[b].min() <= 0.0:                                             # exactly decomposed: the 7x7 system is singular
+            continue
+        try:
+            ex = _backward_exact_mp(P[b], G[b].astype(np.float64))
+        except ZeroDivisionError:
+            continue
+        worst = max(worst, float(np.abs(ex - dH[b]).max()))
+        checked += 1
+    assert checked >= 60
+    assert worst < 1e-12
+
+
 # ---- P11: every row and column sum of dH vanishes (P(H + a 1^T + 1 b^T) = P(H)) --------------------
 @pytest.mark.parametrize("s", [1.0, 10.0, 100.0])
 def test_backward_row_col_sums_zero(oracle, s):
