@@ -55,12 +55,14 @@ typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
  *             kernel tests the column part |g1|+|g2|+|g3|+|g1+g2+g3|, g = c - 1 (eq. (11)), in fp32
  *             against an internal threshold min(tol, max(tol/2, tol - 5e-7)) that leaves room for the
  *             fp32 rounding of the rows (S3/S9).  tol = 0 runs to the fp32 floor.
- *   max_iter  maximum number of updates of beta per matrix (Newton steps plus fallback column
- *             steps; PAPER.md:319 uses 20).  The start-up Sinkhorn column steps (three for
- *             well-scaled logits, one after the LP start otherwise; S1) are not counted:
- *             function evaluations <= max_iter + 4.  On well-scaled logits the first
- *             min(2, max_iter) updates are taken without testing the residual, so a matrix reports
- *             at least that many updates.
+ *   max_iter  maximum number of updates of beta per matrix (Newton steps plus, in the guarded solver,
+ *             fallback column steps; PAPER.md:319 uses 20).  The start-up steps (three Sinkhorn sweeps
+ *             for well-scaled logits, one balancing step after the LP start otherwise; S1) are
+ *             not counted: function evaluations <= max_iter + 4.  The first min(2, max_iter) updates
+ *             are taken without testing the residual, so a matrix reports at least that many updates.
+ *             A matrix that the lean iteration hands to the guarded solver (S2) is solved again
+ *             with the updates that are left, and reports the sum.  max_iter = 0 is accepted (start
+ *             point only, rows normalised).
  * A matrix that has not converged after max_iter updates gets its last iterate (rows still
  * normalised); this is not an error (Table 2 reports such iterates too).
  */
@@ -77,6 +79,15 @@ int birkhoff4_forward(const float* H, float* P, int64_t B, float tol, int max_it
 int birkhoff4_forward_ex(const float* H, float* P, int64_t B, float tol, int max_iter, int32_t* iters,
                          unsigned long long* hist, unsigned long long* n_unconverged,
                          birkhoff4_stream_t stream);
+
+/*
+ * The guarded solver (residual-decrease guard with Sinkhorn fallback steps, S2) applied to EVERY
+ * matrix instead of only to those the lean iteration leaves: the plain, slower statement of the method, exported
+ * so that the default path can be validated against it.  Same arguments and diagnostics as birkhoff4_forward_ex.
+ */
+int birkhoff4_forward_guarded(const float* H, float* P, int64_t B, float tol, int max_iter, int32_t* iters,
+                              unsigned long long* hist, unsigned long long* n_unconverged,
+                              birkhoff4_stream_t stream);
 
 /* Forward for logits stored as bf16 bit patterns (uint16 [B][4][4], 32 B per matrix); P is fp32. */
 int birkhoff4_forward_bf16(const uint16_t* H, float* P, int64_t B, float tol, int max_iter,
@@ -112,22 +123,15 @@ int birkhoff4_sinkhorn(const float* H, float* P, int64_t B, int n_iter, birkhoff
  *   birkhoff4_backward_host          P_host, dP_host -> dH_host
  *   birkhoff4_forward_backward_host  H_host, dP_host -> P_host (nullable), dH_host
  *                                    (P stays on the device between the two kernels)
+ * The ring belongs to the device that is current when it is first used (a call under another current
+ * device rebuilds it); calls are serialised by a mutex.  On an error the call still waits for every copy
+ * it has started, so no transfer into the caller's buffers is in flight when it returns.
  */
 int birkhoff4_forward_host(const float* H_host, float* P_host, int64_t B, float tol, int max_iter);
 int birkhoff4_backward_host(const float* P_host, const float* dP_host, float* dH_host, int64_t B);
 int birkhoff4_forward_backward_host(const float* H_host, const float* dP_host, float* P_host, float* dH_host,
                                     int64_t B, float tol, int max_iter);
 void birkhoff4_host_release(void);
-
-/*
- * Select the forward kernel variant (for measurement).  Returns the previous value.
- *   0  library default (= 4)
- *   1  guarded solver for every matrix, one matrix per thread
- *   2  guarded solver for every matrix, two matrices per thread (packed FFMA2/FADD2/FMUL2)
- *   3  lean iteration for well-scaled logits + guarded solver for the rest, 3 blocks of 256 threads per SM
- *   4  the same with 4 blocks per SM (64 registers)
- */
-int birkhoff4_set_variant(int variant);
 
 const char* birkhoff4_strerror(int code);
 int birkhoff4_version(void);

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "birkhoff4.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bk4_core.cuh", "bk4_vec.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bk4_math.cuh", "bk4_solve.cuh", "bk4_lean.cuh", "bk4_guarded.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "birkhoff4.h")]
 LIB = os.path.join(HERE, "libbirkhoff4.so")
 
@@ -28,7 +28,8 @@ def nvcc():
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB + ".tmp"] + SOURCES
+    extra = ["-DBK4_EXPERIMENTS"] if os.environ.get("BK4_EXPERIMENTS") else []   # measurement hooks; never in the default build
+    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB + ".tmp"] + SOURCES
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB
