@@ -107,6 +107,16 @@ int birkhoff4_forward_bf16_ex(const uint16_t* H, float* P, int64_t B, float tol,
 int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, birkhoff4_stream_t stream);
 
 /*
+ * Fused forward + backward for recompute-style training (the backward needs nothing of the
+ * forward but its result): one kernel projects H and differentiates the result while it is still in registers.
+ * H, dP = dL/dP, dH = dL/dH: device fp32 [B][4][4]; P: device fp32 [B][4][4] or NULL (then the projection is never
+ * written: 64 + 64 bytes in and 64 out per matrix instead of the 320 of the two separate calls).  Aliases allowed:
+ * dH == dP, P == H.  P and dH are bit-identical to birkhoff4_forward followed by birkhoff4_backward.
+ */
+int birkhoff4_forward_backward(const float* H, const float* dP, float* P, float* dH, int64_t B, float tol, int max_iter,
+                               birkhoff4_stream_t stream);
+
+/*
  * Sinkhorn-Knopp baseline (eq. (2)): K = exp(H) (row-max shifted, which the first row
  * normalisation cancels), then n_iter x (rows /= row sums; columns /= column sums).  n_iter = 20 is the
  * "Sinkhorn-20" of PAPER.md:32, 319.  Reported baseline only.

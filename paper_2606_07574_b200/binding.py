@@ -40,6 +40,7 @@ def lib():
             "forward_bf16": [vp, vp, i64, f32, ci, vp],
             "forward_bf16_ex": [vp, vp, i64, f32, ci, vp, vp, vp, vp],
             "backward": [vp, vp, vp, i64, vp],
+            "forward_backward": [vp, vp, vp, vp, i64, f32, ci, vp],
             "sinkhorn": [vp, vp, i64, ci, vp],
             "forward_host": [vp, vp, i64, f32, ci],
             "backward_host": [vp, vp, vp, i64],
@@ -169,6 +170,20 @@ def birkhoff4_backward(P, dP, dH=None, stream=None):
     with torch.cuda.device(P.device):
         _check(lib().birkhoff4_backward(_ptr(P), _ptr(dP), _ptr(dH), B, _stream(stream, P.device)))
     return dH
+
+
+def birkhoff4_forward_backward(H, dP, P=None, dH=None, tol=1e-6, max_iter=20, want_P=True, stream=None):
+    """fused forward + backward (one kernel): returns (P or None, dH); P is not written when want_P is False"""
+    H = _dev(H, torch.float32, "H")
+    B = _batch(H, 16, "H")
+    dP = _dev(dP, torch.float32, "dP", H.numel(), H)
+    if want_P or P is not None:
+        P = _out(P, H, "P")
+    dH = _out(dH, H, "dH")
+    with torch.cuda.device(H.device):
+        _check(lib().birkhoff4_forward_backward(_ptr(H), _ptr(dP), _ptr(P), _ptr(dH), B, tol, max_iter,
+                                                _stream(stream, H.device)))
+    return P, dH
 
 
 def birkhoff4_sinkhorn(H, P=None, n_iter=20, stream=None):

@@ -15,7 +15,8 @@
 
 namespace bk4 {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = BK4_THREADS;  // forward kernels
+constexpr int kThreadsBwd = 256;       // backward and Sinkhorn kernels
 static_assert(kThreads == kSmStride, "the scratch column stride is the block size");
 
 // largest in-row logit range max_i (max_j H_ij - min_j H_ij) up to which a matrix starts from beta = 0 (above: LP
@@ -52,9 +53,16 @@ static cudaError_t launch(void (*kernel)(KArgs...), unsigned grid, unsigned bloc
 // guarded solver afterwards, in a branch a warp skips when it has none.  A matrix's result depends on that matrix
 // alone, not on which matrices share its warp.
 // GUARDED_ONLY (birkhoff4_forward_guarded): the lean part is skipped and every matrix takes the guarded solver.
-template <bool BF16, bool DIAG, bool GUARDED_ONLY = false>
-__global__ void __launch_bounds__(kThreads, 4) forward_kernel(const void* __restrict__ H, float* __restrict__ P, int64_t B,
-                                                              float tol_i, int max_iter, float lp_range, FwdDiag diag) {
+// FUSED_BWD (birkhoff4_forward_backward): the backward pass runs on the result while it is still in
+// registers: dH from P and dP = dL/dP; P itself is written only if the pointer is not null.
+struct FusedBwd {
+    const float* dP;
+    float* dH;
+};
+template <bool BF16, bool DIAG, bool GUARDED_ONLY = false, bool FUSED_BWD = false>
+__global__ void __launch_bounds__(kThreads, 1024 / kThreads) forward_kernel(const void* __restrict__ H, float* __restrict__ P, int64_t B,
+                                                              float tol_i, int max_iter, float lp_range, FwdDiag diag,
+                                                              FusedBwd bwd) {
     pdl_wait_and_trigger();
     __shared__ float s_col[16 * kThreads];
     __shared__ unsigned int s_hist[DIAG ? BIRKHOFF4_HIST_BINS : 1];
@@ -73,6 +81,16 @@ __global__ void __launch_bounds__(kThreads, 4) forward_kernel(const void* __rest
             if (diag.iters) diag.iters[idx] = iters;
             atomicAdd(&s_hist[min(iters, BIRKHOFF4_HIST_BINS - 1)], 1u);
             if (!converged) atomicAdd(&s_unc, 1u);
+        }
+    };
+    // the result of this thread's matrix (original column order): store it and, when fused, differentiate it
+    auto commit = [&](const float(&out)[16]) {
+        if (!FUSED_BWD || P) store_matrix(P + 16 * idx, out);
+        if constexpr (FUSED_BWD) {
+            float g[16], d[16];
+            load_matrix(bwd.dP + 16 * idx, g);  // dH may alias dP: coherent load
+            backward_ift(out, g, d);
+            store_matrix(bwd.dH + 16 * idx, d);
         }
     };
     bool left = valid;  // this thread's matrix still has to be solved
@@ -119,11 +137,11 @@ __global__ void __launch_bounds__(kThreads, 4) forward_kernel(const void* __rest
                 if (active && res.stored) {
                     float out[16];
                     unpermute_columns(T, code, sm, out);
-                    store_matrix(P + 16 * idx, out);
+                    commit(out);
                 }
             } else {
                 res = lean_iterate(E, v0, v1, v2, active, tol_i, max_iter, T);
-                if (active && res.stored) store_matrix(P + 16 * idx, T);
+                if (active && res.stored) commit(T);
             }
             if (active && res.stored) record(res.it, res.converged);
             left = valid && !(active && res.stored);
@@ -156,7 +174,7 @@ __global__ void __launch_bounds__(kThreads, 4) forward_kernel(const void* __rest
                 unpermute_columns(T, code, sm, out);
 #pragma unroll
                 for (int q = 0; q < 16; ++q) out[q] = bad ? kNaN : out[q];
-                store_matrix(P + 16 * idx, out);
+                commit(out);
                 record(it_lean + iters, converged && !bad);
             };
             newton_guarded(hc, xs, tol_i, max_iter > it_lean ? max_iter - it_lean : 0, gather, emit);
@@ -171,7 +189,7 @@ __global__ void __launch_bounds__(kThreads, 4) forward_kernel(const void* __rest
 }
 
 // ---------------------------------------------------------------- backward kernel (HBM-bound: 192 B per matrix)
-__global__ void __launch_bounds__(kThreads) backward_kernel(const float* __restrict__ P, const float* __restrict__ dP,
+__global__ void __launch_bounds__(kThreadsBwd) backward_kernel(const float* __restrict__ P, const float* __restrict__ dP,
                                                             float* __restrict__ dH, int64_t B) {
     pdl_wait_and_trigger();
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -184,7 +202,7 @@ __global__ void __launch_bounds__(kThreads) backward_kernel(const float* __restr
 }
 
 // ---------------------------------------------------------------- Sinkhorn-Knopp baseline kernel
-__global__ void __launch_bounds__(kThreads) sinkhorn_kernel(const float* __restrict__ H, float* __restrict__ P, int64_t B,
+__global__ void __launch_bounds__(kThreadsBwd) sinkhorn_kernel(const float* __restrict__ H, float* __restrict__ P, int64_t B,
                                                             int n_iter) {
     pdl_wait_and_trigger();
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -198,7 +216,7 @@ __global__ void __launch_bounds__(kThreads) sinkhorn_kernel(const float* __restr
 // ---------------------------------------------------------------- host side
 static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) != 0; }
 static inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? BIRKHOFF4_OK : BIRKHOFF4_ECUDA_BASE + (int)e; }
-static inline unsigned grid_for(int64_t B) { return (unsigned)((B + kThreads - 1) / kThreads); }
+static inline unsigned grid_for(int64_t B, int threads) { return (unsigned)((B + threads - 1) / threads); }
 
 // The kernels test the column residual err = sum_m |g_m| computed in fp32 (rows sum to 1 by construction).  Err of
 // PAPER.md:323, evaluated exactly on the stored fp32 P, adds to it the rounding of the stored entries (up to half an
@@ -212,12 +230,13 @@ static inline float internal_tol(float tol) {
     return fmaxf(f * tol, tol - 7e-7f);
 }
 
-template <bool BF16, bool GUARDED_ONLY = false>
+template <bool BF16, bool GUARDED_ONLY = false, bool FUSED_BWD = false>
 static int launch_forward(const void* H, float* P, int64_t B, float tol, int max_iter, FwdDiag diag,
-                          cudaStream_t stream) {
+                          cudaStream_t stream, FusedBwd bwd = FusedBwd{nullptr, nullptr}) {
     if (B < 0 || !(tol >= 0.0f) || max_iter < 0) return BIRKHOFF4_EINVAL;
     if (B == 0) return BIRKHOFF4_OK;
-    if (!H || !P || misaligned(H) || misaligned(P)) return BIRKHOFF4_EINVAL;
+    if (!H || misaligned(H) || misaligned(P) || (!P && !FUSED_BWD)) return BIRKHOFF4_EINVAL;
+    if (FUSED_BWD && (!bwd.dP || !bwd.dH || misaligned(bwd.dP) || misaligned(bwd.dH))) return BIRKHOFF4_EINVAL;
     const bool want_diag = diag.iters || diag.hist || diag.n_unconverged;
     const float tol_i = internal_tol(tol);
     cudaError_t rc;
@@ -227,9 +246,11 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
     const float lpr = kLpRange;
 #endif
     if (want_diag)
-        rc = launch(forward_kernel<BF16, true, GUARDED_ONLY>, grid_for(B), kThreads, stream, H, P, B, tol_i, max_iter, lpr, diag);
+        rc = launch(forward_kernel<BF16, true, GUARDED_ONLY, FUSED_BWD>, grid_for(B, kThreads), kThreads, stream, H, P, B, tol_i,
+                    max_iter, lpr, diag, bwd);
     else
-        rc = launch(forward_kernel<BF16, false, GUARDED_ONLY>, grid_for(B), kThreads, stream, H, P, B, tol_i, max_iter, lpr, diag);
+        rc = launch(forward_kernel<BF16, false, GUARDED_ONLY, FUSED_BWD>, grid_for(B, kThreads), kThreads, stream, H, P, B, tol_i,
+                    max_iter, lpr, diag, bwd);
     return cuda_rc(rc);
 }
 
@@ -354,18 +375,24 @@ int birkhoff4_forward_guarded(const float* H, float* P, int64_t B, float tol, in
     return launch_forward<false, true>(H, P, B, tol, max_iter, FwdDiag{iters, hist, n_unconverged}, (cudaStream_t)stream);
 }
 
+int birkhoff4_forward_backward(const float* H, const float* dP, float* P, float* dH, int64_t B, float tol, int max_iter,
+                               birkhoff4_stream_t stream) {
+    return launch_forward<false, false, true>(H, P, B, tol, max_iter, FwdDiag{nullptr, nullptr, nullptr}, (cudaStream_t)stream,
+                                              FusedBwd{dP, dH});
+}
+
 int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, birkhoff4_stream_t stream) {
     if (B < 0) return BIRKHOFF4_EINVAL;
     if (B == 0) return BIRKHOFF4_OK;
     if (!P || !dP || !dH || misaligned(P) || misaligned(dP) || misaligned(dH)) return BIRKHOFF4_EINVAL;
-    return cuda_rc(launch(backward_kernel, grid_for(B), kThreads, (cudaStream_t)stream, P, dP, dH, B));
+    return cuda_rc(launch(backward_kernel, grid_for(B, kThreadsBwd), kThreadsBwd, (cudaStream_t)stream, P, dP, dH, B));
 }
 
 int birkhoff4_sinkhorn(const float* H, float* P, int64_t B, int n_iter, birkhoff4_stream_t stream) {
     if (B < 0 || n_iter < 0) return BIRKHOFF4_EINVAL;
     if (B == 0) return BIRKHOFF4_OK;
     if (!H || !P || misaligned(H) || misaligned(P)) return BIRKHOFF4_EINVAL;
-    return cuda_rc(launch(sinkhorn_kernel, grid_for(B), kThreads, (cudaStream_t)stream, H, P, B, n_iter));
+    return cuda_rc(launch(sinkhorn_kernel, grid_for(B, kThreadsBwd), kThreadsBwd, (cudaStream_t)stream, H, P, B, n_iter));
 }
 
 int birkhoff4_forward_host(const float* H_host, float* P_host, int64_t B, float tol, int max_iter) {

@@ -596,3 +596,48 @@ def test_host_calls_match_device_calls(B):
     _, dH3 = bk.birkhoff4_forward_backward_host(torch.from_numpy(H), torch.from_numpy(G), want_P=False)   # pageable
     assert torch.equal(dH3, dH.cpu())
     bk.birkhoff4_host_release()
+
+
+# ---------------------------------------------------------------------------------------------------
+# fused forward + backward: bit-identical to the two separate calls
+@pytest.mark.parametrize("s", [1.0, 30.0])
+@pytest.mark.parametrize("B", [1, 33, 1000, 70001])
+def test_fused_forward_backward_equals_separate_calls(oracle, B, s):
+    H, G = inputs.normal(B, s, config=90, sub=B)
+    Hd, Gd = dev(H), dev(G)
+    P = bk.birkhoff4_forward(Hd, max_iter=32)
+    dH = bk.birkhoff4_backward(P, Gd)
+    # guard cells: nothing is written past B matrices
+    pbuf, dbuf = torch.full((B + 2, 4, 4), 7.0, device="cuda"), torch.full((B + 2, 4, 4), 7.0, device="cuda")
+    bk.birkhoff4_forward_backward(Hd, Gd, pbuf[1:B + 1], dbuf[1:B + 1], max_iter=32)
+    assert torch.equal(pbuf[1:B + 1], P) and torch.equal(dbuf[1:B + 1], dH)
+    for buf in (pbuf, dbuf):
+        assert (host(buf[0]) == 7.0).all() and (host(buf[B + 1]) == 7.0).all()
+    none, dH2 = bk.birkhoff4_forward_backward(Hd, Gd, want_P=False, max_iter=32)    # P never written
+    assert none is None and torch.equal(dH2, dH)
+    X, Y = Hd.clone(), Gd.clone()
+    bk.birkhoff4_forward_backward(X, Y, X, Y, max_iter=32)                          # P == H and dH == dP
+    assert torch.equal(X, P) and torch.equal(Y, dH)
+    if B >= 1000:                                                                   # and against the oracle
+        P_o = oracle.forward(H.astype(np.float64))
+        e1, e2 = dh_errors(host(dH2).astype(np.float64), oracle.backward(P_o, G.astype(np.float64)), G)
+        assert e1 <= TOL_DH and e2 <= TOL_DH
+
+
+def test_fused_forward_backward_mixed_and_nonfinite():
+    H = _mixed_batch(8192, seed=91)
+    H[5::64, 0, 1] = np.nan
+    G = np.random.default_rng(92).normal(size=H.shape).astype(np.float32)
+    Hd, Gd = dev(H), dev(G)
+    P = bk.birkhoff4_forward(Hd, max_iter=32)
+    dH = bk.birkhoff4_backward(P, Gd)
+    P2, dH2 = bk.birkhoff4_forward_backward(Hd, Gd, max_iter=32)
+    assert torch.equal(torch.nan_to_num(P2, nan=-1.0), torch.nan_to_num(P, nan=-1.0))
+    assert torch.equal(torch.nan_to_num(dH2, nan=-1.0), torch.nan_to_num(dH, nan=-1.0))
+    assert bool(torch.isnan(P2[5::64]).all()) and bool(torch.isfinite(P2[6::64]).all())
+    L = bk.lib()
+    import ctypes
+    p = ctypes.c_void_p(Hd.data_ptr())
+    assert L.birkhoff4_forward_backward(p, None, p, p, 4, 1e-6, 20, None) == 1       # dP missing
+    assert L.birkhoff4_forward_backward(p, p, None, None, 4, 1e-6, 20, None) == 1    # dH missing
+    assert L.birkhoff4_forward_backward(None, None, None, None, 0, 1e-6, 20, None) == 0
