@@ -23,5 +23,21 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+SRC_OT = os.path.join(HERE, "ot_oracle.c")
+LIB_OT = os.path.join(HERE, "libot_oracle.so")
+
+
+def build_ot(force: bool = False) -> str:
+    """the general small entropic-OT / n x n Birkhoff oracle (oracle/ot_oracle.c)"""
+    if not force and os.path.exists(LIB_OT) and os.path.getmtime(LIB_OT) >= os.path.getmtime(SRC_OT):
+        return LIB_OT
+    cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-Wall", "-Wextra",
+           "-o", LIB_OT + ".tmp", SRC_OT, "-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(LIB_OT + ".tmp", LIB_OT)
+    return LIB_OT
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv))
+    print(build_ot(force="--force" in sys.argv))

@@ -62,6 +62,34 @@ def uniform(B, half_width=1.0, config=0, sub=0):
     return H, G
 
 
+def normal_n(B, n, scale=1.0, config=8, sub=0):
+    """H, G for the n x n Birkhoff projection (n = 4 or 8): H ~ N(0, scale^2), G ~ N(0,1), fp32 [B,n,n]."""
+    rng = _rng(config, sub)
+    H = rng.standard_normal((B, n, n), dtype=np.float32)
+    if scale != 1.0:
+        H *= np.float32(scale)
+    G = rng.standard_normal((B, n, n), dtype=np.float32)
+    return H, G
+
+
+def ot_problem(B, n, m, scale=1.0, config=9, sub=0, uniform_marginals=False):
+    """A batch of small entropic-OT problems: cost M ~ N(0, scale^2) [B,n,m], marginals a [B,n] and
+    b [B,m] positive with equal sums (Gamma(4) draws, rescaled so that sum a = sum b = max(n, m); all ones when
+    uniform_marginals and n == m), upstream gradient G ~ N(0,1).  All fp32; b is rescaled in fp64 and rounded, so the
+    two sums agree to fp32 rounding."""
+    rng = _rng(config, sub)
+    M = (rng.standard_normal((B, n, m), dtype=np.float32) * np.float32(scale)).astype(np.float32)
+    G = rng.standard_normal((B, n, m), dtype=np.float32)
+    if uniform_marginals and n == m:
+        return M, np.ones((B, n), np.float32), np.ones((B, m), np.float32), G
+    a = rng.gamma(4.0, size=(B, n))
+    b = rng.gamma(4.0, size=(B, m))
+    tot = float(max(n, m))
+    a = (a * (tot / a.sum(1, keepdims=True))).astype(np.float32)
+    b = (b * (a.astype(np.float64).sum(1, keepdims=True) / b.sum(1, keepdims=True))).astype(np.float32)
+    return M, a, b, G
+
+
 def heterogeneous(B, config=5, sub=0, sort_by_class=False):
     """config 5.  Returns H, G, cls (0 scaled normal, 1 near-permutation, 2 duplicate row, 3 ties)."""
     rng = _rng(config, sub)
