@@ -50,6 +50,11 @@ def lib():
         for name, args in sig.items():
             f = getattr(L, "birkhoff4_" + name)
             f.argtypes, f.restype = args, ci
+        L.birkhoff8_forward.argtypes, L.birkhoff8_forward.restype = [vp, vp, i64, f32, ci, vp, vp, vp], ci
+        L.birkhoff8_backward.argtypes, L.birkhoff8_backward.restype = [vp, vp, vp, i64, vp], ci
+        L.entropic_ot_forward.argtypes = [vp, vp, vp, vp, i64, ci, ci, f32, f32, ci, vp, vp, vp]
+        L.entropic_ot_forward.restype = ci
+        L.entropic_ot_backward.argtypes, L.entropic_ot_backward.restype = [vp, vp, vp, i64, ci, ci, f32, vp], ci
         L.birkhoff4_host_release.argtypes = []
         L.birkhoff4_host_release.restype = None
         L.birkhoff4_strerror.argtypes = [ci]
@@ -224,6 +229,69 @@ def birkhoff4_forward_backward_host(H_host, dP_host, P_host=None, dH_host=None, 
     _check(lib().birkhoff4_forward_backward_host(_ptr(H_host), _ptr(dP_host), _ptr(P_host), _ptr(dH_host),
                                                  H_host.numel() // 16, tol, max_iter))
     return P_host, dH_host
+
+
+# ------------------------------------------------------------------------------ include/birkhoff_ot.h
+def birkhoff8_forward(H, P=None, tol=2e-6, max_iter=40, iters=None, n_unconverged=None, stream=None):
+    """n = 8 Birkhoff projection of exp(H), fp32 CUDA H[B,8,8]"""
+    H = _dev(H, torch.float32, "H")
+    B = _batch(H, 64, "H")
+    P = _out(P, H, "P")
+    if iters is not None:
+        _dev(iters, torch.int32, "iters", B, H)
+    if n_unconverged is not None:
+        _dev(n_unconverged, torch.int64, "n_unconverged", 1, H)
+    with torch.cuda.device(H.device):
+        _check(lib().birkhoff8_forward(_ptr(H), _ptr(P), B, tol, max_iter, _ptr(iters), _ptr(n_unconverged),
+                                       _stream(stream, H.device)))
+    return P
+
+
+def birkhoff8_backward(P, dP, dH=None, stream=None):
+    """dH = dL/dH from P and dP = dL/dP for the n = 8 projection (fp32 CUDA [B,8,8])"""
+    P = _dev(P, torch.float32, "P")
+    B = _batch(P, 64, "P")
+    dP = _dev(dP, torch.float32, "dP", P.numel(), P)
+    dH = _out(dH, P, "dH")
+    with torch.cuda.device(P.device):
+        _check(lib().birkhoff8_backward(_ptr(P), _ptr(dP), _ptr(dH), B, _stream(stream, P.device)))
+    return dH
+
+
+def entropic_ot_forward(C, a=None, b=None, T=None, eta=1.0, tol=2e-6, max_iter=40, iters=None, n_unconverged=None,
+                        stream=None):
+    """T = argmin <T,C> - eta h(T) over Pi(a,b) for fp32 CUDA costs C[B,n,m], marginals a[B,n], b[B,m] (or both None)"""
+    C = _dev(C, torch.float32, "C")
+    if C.dim() != 3:
+        raise Birkhoff4Error("C must be [B,n,m]")
+    B, n, m = C.shape
+    if (a is None) != (b is None):
+        raise Birkhoff4Error("give both marginals or neither")
+    if a is not None:
+        a = _dev(a, torch.float32, "a", B * n, C)
+        b = _dev(b, torch.float32, "b", B * m, C)
+    T = _out(T, C, "T")
+    if iters is not None:
+        _dev(iters, torch.int32, "iters", B, C)
+    if n_unconverged is not None:
+        _dev(n_unconverged, torch.int64, "n_unconverged", 1, C)
+    with torch.cuda.device(C.device):
+        _check(lib().entropic_ot_forward(_ptr(C), _ptr(a), _ptr(b), _ptr(T), B, n, m, eta, tol, max_iter, _ptr(iters),
+                                         _ptr(n_unconverged), _stream(stream, C.device)))
+    return T
+
+
+def entropic_ot_backward(T, G, D=None, eta=1.0, stream=None):
+    """D = dl/dC from the forward output T and G = dl/dT (eq. (13)), fp32 CUDA [B,n,m]"""
+    T = _dev(T, torch.float32, "T")
+    if T.dim() != 3:
+        raise Birkhoff4Error("T must be [B,n,m]")
+    B, n, m = T.shape
+    G = _dev(G, torch.float32, "G", T.numel(), T)
+    D = _out(D, T, "D")
+    with torch.cuda.device(T.device):
+        _check(lib().entropic_ot_backward(_ptr(T), _ptr(G), _ptr(D), B, n, m, eta, _stream(stream, T.device)))
+    return D
 
 
 def birkhoff4_host_release():

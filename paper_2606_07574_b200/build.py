@@ -9,9 +9,9 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = [os.path.join(CSRC, "birkhoff4.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bk4_math.cuh", "bk4_solve.cuh", "bk4_lean.cuh", "bk4_guarded.cuh")] + [
-    os.path.join(os.path.dirname(HERE), "include", "birkhoff4.h")]
+SOURCES = [os.path.join(CSRC, "birkhoff4.cu"), os.path.join(CSRC, "birkhoff_ot.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bk4_math.cuh", "bk4_solve.cuh", "bk4_lean.cuh", "bk4_guarded.cuh", "bk_ot.cuh")] + [
+    os.path.join(os.path.dirname(HERE), "include", f) for f in ("birkhoff4.h", "birkhoff_ot.h")]
 LIB = os.path.join(HERE, "libbirkhoff4.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-ftz=true",

@@ -1,0 +1,367 @@
+// bk_ot.cuh -- small entropic-regularised optimal transport, N x M with N, M <= 8, one problem per thread: the
+// general problem of PAPER.md section 2.3 / 3.1 of which the 4x4 Birkhoff projection is the special case, and in
+// particular the n = 8 Birkhoff projection.  SURVEY.md 8(f) NEXT-1 and NEXT-3.
+//
+//   forward   T = argmin_{T in Pi(a,b)} <T, C> - eta h(T)   (eq. (3)) by Newton's method on the
+//             (M-1)-variable dual f(beta_{-M}) (eq. (8)) with gradient and Hessian of eq. (9)
+//             PAPER.md:144-147, T_i. = a_i Softmax(U_i. / eta), a guarded step
+//             and a stop on the marginal error (PAPER.md:323 with the marginals a, b).
+//   backward  D = dl/dC from T and G = dl/dT by eq. (13) PAPER.md:273-280.
+//
+// What is the same as in the 4x4 kernels (bk4_*.cuh): incremental exponentials (E = exp(U0/eta - mu) once per
+// base point, v_j = exp(delta_j/eta), a Newton update is v_j *= exp(d_j)); the Hessian written as the Laplacian of
+// the column graph with edge weights W_jk = sum_i T_ij T_ik / a_i, grounded at column M and solved by node
+// elimination (every pivot a sum of non-negative terms; S7); the residual-decrease guard with a
+// Sinkhorn column step as fallback (S2).
+// What is different: rows are streamed (T is never held whole: with N M = 64 entries the registers hold E, the
+// column sums and the M(M-1)/2 edge weights); there is no LP start (an assignment problem for N = M = 8 has no
+// 24-permutation brute force): wide costs are reached by continuation in eta (eps-scaling): the problem is solved
+// at eta 2^K, ..., 2 eta, eta with 2^K eta ~ range / 8, each stage started from the potentials of the one before.
+#pragma once
+#include "bk4_math.cuh"
+
+namespace bkot {
+
+using namespace bk4;
+
+constexpr float kOtLam = 2.384185791015625e-07f;  // ground regularisation, relative to the mean row marginal
+constexpr int kOtSweeps = 3;                     // Sinkhorn sweeps at the start of every continuation stage
+constexpr float kOtStageRange = 8.0f;            // a stage's scaled costs span at most this
+constexpr int kOtHalvings = 4;                   // step halvings before the Sinkhorn fallback
+constexpr float kOtStageTol = 1e-2f;             // relative marginal error at which an intermediate stage is left
+
+// vector load/store of one row of K floats (K = 4: 128 bits, K = 8: 256 bits, else scalar)
+template <int K>
+BK4_DEV void load_row(const float* p, float (&r)[K]) {
+    if constexpr (K == 8) {
+        ld256(p, r);
+    } else if constexpr (K == 4) {
+        const float4 t = *reinterpret_cast<const float4*>(p);
+        r[0] = t.x, r[1] = t.y, r[2] = t.z, r[3] = t.w;
+    } else {
+#pragma unroll
+        for (int j = 0; j < K; ++j) r[j] = p[j];
+    }
+}
+template <int K>
+BK4_DEV void store_row(float* p, const float (&r)[K]) {
+    if constexpr (K == 8) {
+        stg256(p, r);
+    } else if constexpr (K == 4) {
+        *reinterpret_cast<float4*>(p) = make_float4(r[0], r[1], r[2], r[3]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < K; ++j) p[j] = r[j];
+    }
+}
+
+// index of the edge weight W_jk, j < k < M, in the packed upper triangle
+template <int M>
+BK4_DEV constexpr int tri(int j, int k) {
+    return j * M - j * (j + 1) / 2 + (k - j - 1);
+}
+
+// Solve the grounded Laplacian system L d = -g, L_jk = -W_jk (j != k), L_jj = sum_{k != j} W_jk, unknowns j < M-1,
+// ground = column M-1 (its links get `lam`), by node elimination in the order 0, 1, ...  W (packed) is destroyed.
+template <int M>
+BK4_DEV void solve_laplacian(float (&W)[M * (M - 1) / 2], const float (&g)[M], float lam, float (&d)[M - 1]) {
+    constexpr int K = M - 1;
+    float deg[K], rhs[K], inv[K];
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+        W[tri<M>(j, K)] += lam;
+        float s = 0.0f;
+#pragma unroll
+        for (int k = 0; k < M; ++k)
+            if (k != j) s += W[k > j ? tri<M>(j, k) : tri<M>(k, j)];
+        deg[j] = s;
+        rhs[j] = -g[j];
+    }
+    // eliminate node p: for its neighbours j, k > p:  W_jk += W_pj W_pk / deg_p,  deg_j -= W_pj - (W_pj / deg_p)(deg_p - W_pj) ...
+    // written through the degrees: deg_j' = sum of the new weights of j, which is deg_j - W_pj^2 / deg_p  (the link
+    // to p goes, the links it gains sum to W_pj (deg_p - W_pj) / deg_p)
+#pragma unroll
+    for (int p = 0; p < K; ++p) {
+        inv[p] = rcp_approx(deg[p]);
+#pragma unroll
+        for (int j = p + 1; j < K; ++j) {
+            const float f = W[tri<M>(p, j)] * inv[p];
+#pragma unroll
+            for (int k = j + 1; k < M; ++k) W[tri<M>(j, k)] = fmaf(f, W[tri<M>(p, k)], W[tri<M>(j, k)]);
+            // new degree of j: recomputed from non-negative terms below (no subtraction)
+            rhs[j] = fmaf(f, rhs[p], rhs[j]);
+        }
+#pragma unroll
+        for (int j = p + 1; j < K; ++j) {
+            // links of j to the nodes before it are gone; its degree is the sum over what is left plus what it gained
+            // through p: sum_{k > p, k != j} W'_jk.  The weights W'_jk for k < j were updated symmetrically above
+            // (stored at tri(k, j)), so the sum runs over the packed triangle.
+            float s = 0.0f;
+#pragma unroll
+            for (int k = p + 1; k < M; ++k)
+                if (k != j) s += W[k > j ? tri<M>(j, k) : tri<M>(k, j)];
+            deg[j] = s;
+        }
+    }
+    // back substitution: d_p = (rhs_p + sum_{k > p, k < K} W_pk d_k) / deg_p
+#pragma unroll
+    for (int p = K - 1; p >= 0; --p) {
+        float s = rhs[p];
+#pragma unroll
+        for (int k = p + 1; k < K; ++k) s = fmaf(W[tri<M>(p, k)], d[k], s);
+        d[p] = s * inv[p];
+    }
+}
+
+// One streamed evaluation at v: column sums c_j = sum_i T_ij, and (HESS) the packed edge weights
+// W_jk = sum_i T_ij T_ik / a_i, with T_ij = a_i E_ij v_j / sum_k E_ik v_k and v_{M-1} = 1.
+template <int N, int M, bool UNIT, bool HESS>
+BK4_DEV void ot_eval(const float (&E)[N * M], const float (&v)[M - 1], const float (&a)[N], float (&c)[M],
+                     float (&W)[M * (M - 1) / 2]) {
+#pragma unroll
+    for (int j = 0; j < M; ++j) c[j] = 0.0f;
+    if constexpr (HESS) {
+#pragma unroll
+        for (int q = 0; q < M * (M - 1) / 2; ++q) W[q] = 0.0f;
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float x[M], s = E[i * M + M - 1];
+        x[M - 1] = s;
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) {
+            x[j] = E[i * M + j] * v[j];
+            s += x[j];
+        }
+        float r = rcp_approx(s);
+        r = fmaf(r, fmaf(-s, r, 1.0f), r);
+        const float ar = UNIT ? r : a[i] * r;
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            x[j] *= ar;  // T_ij
+            c[j] += x[j];
+        }
+        if constexpr (HESS) {
+            const float ia = UNIT ? 1.0f : rcp_approx(a[i]);
+#pragma unroll
+            for (int j = 0; j < M - 1; ++j) {
+                const float tj = UNIT ? x[j] : x[j] * ia;
+#pragma unroll
+                for (int k = j + 1; k < M; ++k) W[tri<M>(j, k)] = fmaf(tj, x[k], W[tri<M>(j, k)]);
+            }
+        }
+    }
+}
+
+// E_ij = exp((beta_j - C_ij) / eta - mu_i) for the base potentials beta (beta_{M-1} = 0), mu_i the row maximum.
+// sign = -1 for costs C (entropic OT), +1 for logits H = -C (Birkhoff projection).  Returns false if a NaN/Inf
+// was met.
+template <int N, int M>
+BK4_DEV bool ot_exponentials(const float* Cg, float sign_over_eta, const float (&beta_over_eta)[M - 1], float (&E)[N * M]) {
+    float poison = 0.0f;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float row[M], u[M];
+        load_row<M>(Cg + i * M, row);
+        float mx = -kInf;
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            poison = __fmaf_rn(row[j], 0.0f, poison);
+            u[j] = j < M - 1 ? fmaf(row[j], sign_over_eta * kLog2e, beta_over_eta[j]) : row[j] * (sign_over_eta * kLog2e);
+            mx = fmaxf(mx, u[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < M; ++j) E[i * M + j] = ex2_approx(u[j] - mx);
+    }
+    return poison == 0.0f;
+}
+
+struct OtStats {
+    int iters;
+    bool converged;
+};
+
+// The whole forward for one problem.  Cg: this problem's N x M costs (or logits) in global memory, a, b: its
+// marginals in registers (ignored when UNIT), T: where the result goes.  tol_rel: the stop threshold on
+// Err_ab / sum(a) ... as an absolute threshold on the column part of Err_ab (rows are exact by construction).
+template <int N, int M, bool UNIT>
+BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const float (&a)[N], const float (&b)[M], float tol_abs,
+                               int max_iter, float* Tg) {
+    float E[N * M], v[M - 1], vprev[M - 1], bl[M - 1], c[M], W[M * (M - 1) / 2];
+    // range of the costs decides the continuation schedule
+    float lo = kInf, hi = -kInf, suma = 0.0f;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float row[M];
+        load_row<M>(Cg + i * M, row);
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            lo = fminf(lo, row[j]);
+            hi = fmaxf(hi, row[j]);
+        }
+        suma += UNIT ? 1.0f : a[i];
+    }
+    const float lam = kOtLam * suma * (1.0f / N);
+    float eta_s = eta;
+    int stages = 0;
+    while ((hi - lo) > kOtStageRange * eta_s && stages < 24) {
+        eta_s *= 2.0f;
+        ++stages;
+    }
+#pragma unroll
+    for (int j = 0; j < M - 1; ++j) bl[j] = 0.0f;  // base potentials / eta_s in log2 units
+    OtStats st = {0, false};
+    bool finite = true;
+    for (;; eta_s *= 0.5f, --stages) {
+        finite = ot_exponentials<N, M>(Cg, sign / eta_s, bl, E) && finite;
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) v[j] = 1.0f;
+        // Sinkhorn sweeps in the scaling form of eq. (2) PAPER.md:76 with marginals: u = a / (E v), v = b / (E^T u)
+        for (int k = 0; k < kOtSweeps; ++k) {
+            ot_eval<N, M, UNIT, false>(E, v, a, c, W);
+            const float t = (UNIT ? 1.0f : b[M - 1]) * rcp_approx(c[M - 1]);
+#pragma unroll
+            for (int j = 0; j < M - 1; ++j) v[j] *= (UNIT ? 1.0f : b[j]) * rcp_approx(c[j] * t);
+        }
+        const float tol_s = stages > 0 ? kOtStageTol * suma : tol_abs;
+        float errprev = kInf, tstep = 1.0f, d[M - 1];
+        unsigned newton_trial = 0u, sink_trial = 0u;
+        int halvings = 0;
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) {
+            vprev[j] = v[j];
+            d[j] = 0.0f;
+        }
+        for (;;) {
+            ot_eval<N, M, UNIT, true>(E, v, a, c, W);
+            float g[M], err = 0.0f;
+#pragma unroll
+            for (int j = 0; j < M; ++j) {
+                g[j] = c[j] - (UNIT ? 1.0f : b[j]);
+                err += fabsf(g[j]);
+            }
+            const bool conv = err <= tol_s;
+            if ((newton_trial | sink_trial) && !(err < errprev) && !conv) {
+                // the trial did not lower the residual (a line search decides the step size):
+                // halve the Newton step up to kOtHalvings times, then a Sinkhorn column step, from the last accepted point
+                if (st.iters < max_iter && newton_trial && halvings < kOtHalvings) {
+                    tstep *= 0.5f;
+                    ++halvings;
+#pragma unroll
+                    for (int j = 0; j < M - 1; ++j) v[j] = vprev[j] * ex2_approx(tstep * d[j]);
+                    ++st.iters;
+                    continue;
+                }
+                if (st.iters < max_iter && newton_trial) {
+                    ot_eval<N, M, UNIT, false>(E, vprev, a, c, W);
+                    const float t = (UNIT ? 1.0f : b[M - 1]) * rcp_approx(c[M - 1]);
+#pragma unroll
+                    for (int j = 0; j < M - 1; ++j) v[j] = vprev[j] * ((UNIT ? 1.0f : b[j]) * rcp_approx(c[j] * t));
+                    newton_trial = 0u, sink_trial = 1u;
+                    ++st.iters;
+                    continue;
+                }
+#pragma unroll
+                for (int j = 0; j < M - 1; ++j) v[j] = vprev[j];  // nothing helps (fp32 floor), or no updates left
+                break;
+            }
+            if (conv || !(err == err) || st.iters >= max_iter) {
+                st.converged = conv && stages == 0;
+                break;
+            }
+#pragma unroll
+            for (int j = 0; j < M - 1; ++j) vprev[j] = v[j];
+            errprev = err;
+            solve_laplacian<M>(W, g, lam, d);
+#pragma unroll
+            for (int j = 0; j < M - 1; ++j) {
+                d[j] = fminf(fmaxf(d[j], -30.0f), 30.0f) * kLog2e;  // kept in log2 units for the halvings
+                v[j] *= ex2_approx(d[j]);
+            }
+            tstep = 1.0f, halvings = 0;
+            newton_trial = 1u, sink_trial = 0u;
+            ++st.iters;
+        }
+        if (stages <= 0) break;
+        // next stage: eta halves, so potentials / eta double: beta/eta <- 2 (beta/eta + log2 v)
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) bl[j] = 2.0f * (bl[j] + lg2_approx(v[j]));
+    }
+    // the result: rows at the final v
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float x[M], s = E[i * M + M - 1];
+        x[M - 1] = s;
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) {
+            x[j] = E[i * M + j] * v[j];
+            s += x[j];
+        }
+        float r = rcp_approx(s);
+        r = fmaf(r, fmaf(-s, r, 1.0f), r);
+        const float ar = UNIT ? r : a[i] * r;
+#pragma unroll
+        for (int j = 0; j < M; ++j) x[j] = finite ? x[j] * ar : kNaN;
+        store_row<M>(Tg + i * M, x);
+    }
+    st.converged = st.converged && finite;
+    return st;
+}
+
+// Backward, eq. (13):  Gamma = G o T, mu_r = Gamma 1, mu_c = Gamma^T 1,
+// Delta w = mu_c - T_{-M}^T (mu_r / a), w_M = 0, Delta = diag(c) - T_{-M}^T diag(a)^{-1} T_{-M} as a grounded Laplacian,
+// D_ij = out_scale T_ij ((mu_r_i - (T w)_i) / a_i + w_j - G_ij),  out_scale = 1/eta for dl/dC, -1 for dl/dH of the
+// Birkhoff projection.  The row marginals a are those of the given T.
+template <int N, int M>
+BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, float* Dg) {
+    float T[N * M], G[N * M], W[M * (M - 1) / 2], mur[N], ia[N], rhs[M], w[M - 1];
+#pragma unroll
+    for (int q = 0; q < M * (M - 1) / 2; ++q) W[q] = 0.0f;
+#pragma unroll
+    for (int j = 0; j < M; ++j) rhs[j] = 0.0f;
+    float suma = 0.0f;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float t[M], g[M];
+        load_row<M>(Tg + i * M, t);
+        load_row<M>(Gg + i * M, g);
+        float ai = 0.0f, mr = 0.0f;
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            T[i * M + j] = t[j];
+            G[i * M + j] = g[j];
+            ai += t[j];
+            mr = fmaf(g[j], t[j], mr);
+        }
+        suma += ai;
+        ia[i] = rcp_approx(ai);
+        ia[i] = fmaf(ia[i], fmaf(-ai, ia[i], 1.0f), ia[i]);
+        mur[i] = mr;
+        const float mra = mr * ia[i];
+#pragma unroll
+        for (int j = 0; j < M; ++j) rhs[j] += fmaf(g[j], t[j], -t[j] * mra);  // mu_c_j - sum_i T_ij mu_r_i / a_i
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) {
+            const float tj = t[j] * ia[i];
+#pragma unroll
+            for (int k = j + 1; k < M; ++k) W[tri<M>(j, k)] = fmaf(tj, t[k], W[tri<M>(j, k)]);
+        }
+    }
+    float gneg[M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) gneg[j] = -rhs[j];
+    solve_laplacian<M>(W, gneg, kOtLam * suma * (1.0f / N), w);
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float tw = 0.0f;
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) tw = fmaf(T[i * M + j], w[j], tw);
+        const float vi = (mur[i] - tw) * ia[i];
+        float d[M];
+#pragma unroll
+        for (int j = 0; j < M; ++j) d[j] = out_scale * T[i * M + j] * ((vi - G[i * M + j]) + (j < M - 1 ? w[j] : 0.0f));
+        store_row<M>(Dg + i * M, d);
+    }
+}
+
+}  // namespace bkot

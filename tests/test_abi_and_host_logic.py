@@ -21,15 +21,21 @@ def lib():
     return ctypes.CDLL(build.build())
 
 
+HEADERS = sorted(os.path.join(ROOT, "include", f) for f in os.listdir(os.path.join(ROOT, "include")) if f.endswith(".h"))
+
+
 def declared_symbols():
-    src = open(HEADER).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(birkhoff4_[a-z0-9_]+)\s*\(", src)))
+    """every function declared in include/*.h"""
+    names = set()
+    for h in HEADERS:
+        src = re.sub(r"/\*.*?\*/", "", open(h).read(), flags=re.S)
+        names |= set(re.findall(r"\b((?:birkhoff[0-9]*|entropic_ot|birkhoff_mix)_[a-z0-9_]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_header_compiles_as_plain_c(tmp_path):
     c = tmp_path / "t.c"
-    c.write_text('#include "birkhoff4.h"\nint main(void) { return BIRKHOFF4_OK; }\n')
+    c.write_text("".join('#include "%s"\n' % os.path.basename(h) for h in HEADERS) + "int main(void) { return BIRKHOFF4_OK; }\n")
     subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-c", str(c), "-o",
                     str(tmp_path / "t.o")], check=True)
 
@@ -38,7 +44,8 @@ def test_library_exports_every_declared_symbol(lib):
     names = declared_symbols()
     assert {"birkhoff4_forward", "birkhoff4_backward", "birkhoff4_forward_ex", "birkhoff4_forward_bf16",
             "birkhoff4_sinkhorn", "birkhoff4_forward_backward_host", "birkhoff4_strerror",
-            "birkhoff4_version"} <= set(names)
+            "birkhoff4_version", "birkhoff4_forward_backward", "birkhoff4_forward_guarded", "birkhoff8_forward",
+            "birkhoff8_backward", "entropic_ot_forward", "entropic_ot_backward"} <= set(names)
     for n in names:
         assert hasattr(lib, n), "missing export " + n
 

@@ -1,0 +1,138 @@
+"""GPU parity of the widenings (include/birkhoff_ot.h): the n = 8 Birkhoff projection and small general entropic OT,
+through the C ABI, against the fp64 oracle oracle/ot_oracle.c on the same seeded inputs.
+
+Gates: max |T - T_oracle| <= 1e-5 (relative to the largest marginal), Err_ab <= 2e-6 * sum(a) / 4 ... stated per test,
+D relative error <= 1e-4 (both readings of S10)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+from oracle import ot
+from paper_2606_07574_b200 import binding as bk, inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def host(t):
+    torch.cuda.synchronize()
+    return t.cpu().numpy()
+
+
+def d_errors(D, D_o, G):
+    e1 = np.abs(D - D_o).max() / max(np.abs(D_o).max(), 1e-300)
+    e2 = (np.abs(D - D_o).reshape(len(G), -1).max(1) / np.abs(G).reshape(len(G), -1).max(1)).max()
+    return e1, e2
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-1: n = 8 Birkhoff projection
+@pytest.mark.parametrize("s", [0.1, 1.0, 3.0, 10.0])
+def test_birkhoff8_parity(s):
+    H, G = inputs.normal_n(4096 + 3, 8, s, config=8)
+    P_o, info = ot.forward(-H.astype(np.float64), return_info=True)
+    assert info["uncertified"] == 0
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    it = torch.zeros(len(H), dtype=torch.int32, device="cuda")
+    Pd = bk.birkhoff8_forward(dev(H), tol=2e-6, max_iter=60, iters=it, n_unconverged=unc)
+    P = host(Pd).astype(np.float64)
+    assert np.isfinite(P).all() and P.min() >= 0
+    eP = np.abs(P - P_o).max()
+    err = ot.marginal_err(P)
+    print("birkhoff8 s=%g: eP %.2e Err max %.2e mean %.2e  iters mean %.2f max %d  unconverged %d" % (
+        s, eP, err.max(), err.mean(), float(it.float().mean()), int(it.max()), int(unc.item())))
+    assert eP <= 1e-5
+    assert err.max() <= 2e-6                                          # 16 marginals: twice the 4x4 gate
+    dH = host(bk.birkhoff8_backward(Pd, dev(G))).astype(np.float64)
+    dH_o = ot.birkhoff_backward(P_o, G.astype(np.float64))
+    e1, e2 = d_errors(dH, dH_o, G)
+    assert e1 <= 1e-4 and e2 <= 1e-4, (e1, e2)
+
+
+def test_birkhoff8_properties_and_edges():
+    rng = np.random.default_rng(1)
+    H = (rng.normal(size=(64, 8, 1)) * 4 + rng.normal(size=(64, 1, 8)) * 4).astype(np.float32)
+    P = host(bk.birkhoff8_forward(dev(H)))
+    assert np.abs(P - 0.125).max() < 5e-6                              # separable => uniform (fp32 H is separable up to rounding)
+    H = inputs.normal_n(1000, 8, 1.0, config=8, sub=1)[0]
+    pr, pc = rng.permutation(8), rng.permutation(8)
+    P = host(bk.birkhoff8_forward(dev(H)))
+    Pp = host(bk.birkhoff8_forward(dev(H[:, pr][:, :, pc])))
+    assert np.abs(Pp - P[:, pr][:, :, pc]).max() < 2e-6
+    # ragged sizes, guard cells, NaN isolation, in-place
+    for B in (1, 127, 129, 1000):
+        Hb = H[:B].copy()
+        buf = torch.full((B + 2, 8, 8), 7.0, device="cuda")
+        bk.birkhoff8_forward(dev(Hb), buf[1:B + 1])
+        assert (host(buf[0]) == 7.0).all() and (host(buf[B + 1]) == 7.0).all()
+        assert np.array_equal(host(buf[1:B + 1]), P[:B])
+    Hn = H.copy()
+    Hn[5, 2, 3] = np.nan
+    Hn[6, 0, 0] = np.inf
+    Pn = host(bk.birkhoff8_forward(dev(Hn)))
+    assert np.isnan(Pn[5]).all() and np.isnan(Pn[6]).all()
+    good = np.ones(1000, bool)
+    good[[5, 6]] = False
+    assert np.array_equal(Pn[good], P[good])
+    X = dev(H).clone()
+    bk.birkhoff8_forward(X, X)
+    assert np.array_equal(host(X), P)
+    e = torch.empty((0, 8, 8), device="cuda")
+    assert bk.birkhoff8_forward(e).shape == (0, 8, 8) and bk.birkhoff8_backward(e, e).shape == (0, 8, 8)
+    L = bk.lib()
+    import ctypes
+    p = ctypes.c_void_p(X.data_ptr())
+    assert L.birkhoff8_forward(p, p, -1, 1e-6, 20, None, None, None) == 1
+    assert L.birkhoff8_forward(None, p, 4, 1e-6, 20, None, None, None) == 1
+    assert L.birkhoff8_forward(ctypes.c_void_p(X.data_ptr() + 4), p, 1, 1e-6, 20, None, None, None) == 1
+    assert L.entropic_ot_forward(p, None, None, p, 4, 5, 5, 1.0, 1e-6, 20, None, None, None) == 1     # unsupported size
+    assert L.entropic_ot_forward(p, None, None, p, 4, 4, 8, 1.0, 1e-6, 20, None, None, None) == 1     # unit marginals, n != m
+    assert L.entropic_ot_forward(p, p, None, p, 4, 4, 4, 1.0, 1e-6, 20, None, None, None) == 1        # one marginal missing
+    assert L.entropic_ot_forward(p, None, None, p, 4, 4, 4, 0.0, 1e-6, 20, None, None, None) == 1     # eta = 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-3: general small entropic OT (PAPER.md:83-168 forward, eq. (13) backward)
+@pytest.mark.parametrize("n,m", [(4, 4), (8, 8), (4, 8), (8, 4)])
+@pytest.mark.parametrize("s,eta", [(1.0, 1.0), (3.0, 0.5), (2.0, 2.0), (10.0, 1.0)])
+def test_entropic_ot_parity(n, m, s, eta):
+    Cm, a, b, G = inputs.ot_problem(2048 + 5, n, m, s, config=9, sub=n * 10 + m)
+    # the fp32 marginals' sums agree only to fp32 rounding; problem (3) needs them equal, so the
+    # oracle gets b rescaled in fp64 by 1 + O(1e-7): a perturbation far inside the tolerances below
+    a64, b64 = a.astype(np.float64), b.astype(np.float64)
+    b64 = b64 * (a64.sum(1, keepdims=True) / b64.sum(1, keepdims=True))
+    T_o, info = ot.forward(Cm, a64, b64, eta, return_info=True)
+    assert info["uncertified"] == 0
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    tol = 2e-6 * max(n, m) / 4
+    Td = bk.entropic_ot_forward(dev(Cm), dev(a), dev(b), eta=eta, tol=tol, max_iter=80, n_unconverged=unc)
+    T = host(Td).astype(np.float64)
+    assert np.isfinite(T).all() and T.min() >= 0
+    eT = np.abs(T - T_o).max() / a.max()
+    err = ot.marginal_err(T, a, b)
+    print("ot %dx%d s=%g eta=%g: eT %.2e Err max %.2e  unconverged %d" % (n, m, s, eta, eT, err.max(), int(unc.item())))
+    assert eT <= 1e-5
+    # the marginals given in fp32 do not have exactly equal sums: that mismatch is part of Err_ab and not the solver's
+    mism = np.abs(a.astype(np.float64).sum(1) - b.astype(np.float64).sum(1)).max()
+    assert err.max() <= tol + mism + 1e-6
+    D = host(bk.entropic_ot_backward(Td, dev(G), eta=eta)).astype(np.float64)
+    D_o = ot.backward(T_o, G.astype(np.float64), eta)
+    e1, e2 = d_errors(D * eta, D_o * eta, G)
+    assert e1 <= 1e-4 and e2 <= 1e-4 * a.max(), (e1, e2)
+
+
+def test_entropic_ot_reduces_to_birkhoff4():
+    """C = -H, eta = 1, unit marginals: the 4x4 Birkhoff projection of the main path"""
+    H, G = inputs.normal(8192, 2.0, config=96)
+    P = host(bk.birkhoff4_forward(dev(H)))
+    T = host(bk.entropic_ot_forward(dev(-H), tol=1e-6, max_iter=40))
+    assert np.abs(T - P).max() < 2e-6
+    dH = host(bk.birkhoff4_backward(dev(P), dev(G)))
+    D = host(bk.entropic_ot_backward(dev(P), dev(G)))
+    assert np.abs(D + dH).max() < 5e-6
+    T8 = host(bk.entropic_ot_forward(dev(-inputs.normal_n(512, 8, 1.0, config=97)[0])))
+    P8 = host(bk.birkhoff8_forward(dev(inputs.normal_n(512, 8, 1.0, config=97)[0])))
+    assert np.array_equal(T8, P8)
