@@ -117,6 +117,20 @@ int birkhoff4_forward_backward(const float* H, const float* dP, float* P, float*
                                birkhoff4_stream_t stream);
 
 /*
+ * Fused consumer: the residual-stream mix of PAPER.md:46-50 with its mixing matrix
+ * projected in the same kernel,
+ *     Y_b = P_b X_b,   P_b = proj^KL_{B_4}(exp(H_b)),   b = 0..B-1 (tokens),
+ * X, Y: device [B][4][C] row-major (stream j of token b at (4 b + j) C), fp32 or bf16 bit patterns (fp32
+ * accumulation, round-to-nearest-even on store); C a multiple of 4 (fp32) or 8 (bf16); X, Y 16-byte aligned; Y must
+ * not alias X.  P: device fp32 [B][4][4] or NULL: written only if given (the backward pass needs it).  P never
+ * makes the round trip through HBM that birkhoff4_forward followed by a separate mix pays.
+ */
+int birkhoff4_forward_mix(const float* H, const float* X, float* Y, float* P, int64_t B, int C, float tol, int max_iter,
+                          birkhoff4_stream_t stream);
+int birkhoff4_forward_mix_bf16(const float* H, const uint16_t* X, uint16_t* Y, float* P, int64_t B, int C, float tol,
+                               int max_iter, birkhoff4_stream_t stream);
+
+/*
  * Sinkhorn-Knopp baseline (eq. (2)): K = exp(H) (row-max shifted, which the first row
  * normalisation cancels), then n_iter x (rows /= row sums; columns /= column sums).  n_iter = 20 is the
  * "Sinkhorn-20" of PAPER.md:32, 319.  Reported baseline only.

@@ -41,6 +41,8 @@ def lib():
             "forward_bf16_ex": [vp, vp, i64, f32, ci, vp, vp, vp, vp],
             "backward": [vp, vp, vp, i64, vp],
             "forward_backward": [vp, vp, vp, vp, i64, f32, ci, vp],
+            "forward_mix": [vp, vp, vp, vp, i64, ci, f32, ci, vp],
+            "forward_mix_bf16": [vp, vp, vp, vp, i64, ci, f32, ci, vp],
             "sinkhorn": [vp, vp, i64, ci, vp],
             "forward_host": [vp, vp, i64, f32, ci],
             "backward_host": [vp, vp, vp, i64],
@@ -189,6 +191,25 @@ def birkhoff4_forward_backward(H, dP, P=None, dH=None, tol=1e-6, max_iter=20, wa
         _check(lib().birkhoff4_forward_backward(_ptr(H), _ptr(dP), _ptr(P), _ptr(dH), B, tol, max_iter,
                                                 _stream(stream, H.device)))
     return P, dH
+
+
+def birkhoff4_forward_mix(H, X, Y=None, P=None, tol=1e-6, max_iter=20, want_P=False, stream=None):
+    """fused consumer: Y[b] = proj(exp(H[b])) @ X[b] for X[B,4,C] (fp32 or bfloat16 CUDA); returns (Y, P or None)"""
+    H = _dev(H, torch.float32, "H")
+    B = _batch(H, 16, "H")
+    if not isinstance(X, torch.Tensor) or X.dtype not in (torch.float32, torch.bfloat16):
+        raise Birkhoff4Error("X must be a float32 or bfloat16 tensor")
+    X = _dev(X, X.dtype, "X", like=H)
+    if X.dim() != 3 or X.shape[0] != B or X.shape[1] != 4:
+        raise Birkhoff4Error("X must be [B,4,C]")
+    C = X.shape[2]
+    Y = _out(Y, X, "Y", X.dtype)
+    if want_P or P is not None:
+        P = _out(P, H, "P")
+    fn = lib().birkhoff4_forward_mix if X.dtype == torch.float32 else lib().birkhoff4_forward_mix_bf16
+    with torch.cuda.device(H.device):
+        _check(fn(_ptr(H), _ptr(X), _ptr(Y), _ptr(P), B, C, tol, max_iter, _stream(stream, H.device)))
+    return Y, P
 
 
 def birkhoff4_sinkhorn(H, P=None, n_iter=20, stream=None):

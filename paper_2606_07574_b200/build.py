@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "birkhoff4.cu"), os.path.join(CSRC, "birkhoff_ot.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bk4_math.cuh", "bk4_solve.cuh", "bk4_lean.cuh", "bk4_guarded.cuh", "bk_ot.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bk4_math.cuh", "bk4_solve.cuh", "bk4_lean.cuh", "bk4_guarded.cuh", "bk4_project.cuh", "bk_ot.cuh", "bk4_mix.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", f) for f in ("birkhoff4.h", "birkhoff_ot.h")]
 LIB = os.path.join(HERE, "libbirkhoff4.so")
 

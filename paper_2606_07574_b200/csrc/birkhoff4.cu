@@ -10,8 +10,8 @@
 #include <mutex>
 
 #include "../../include/birkhoff4.h"
-#include "bk4_guarded.cuh"
-#include "bk4_lean.cuh"
+#include "bk4_mix.cuh"
+#include "bk4_project.cuh"
 
 namespace bk4 {
 
@@ -19,9 +19,6 @@ constexpr int kThreads = BK4_THREADS;  // forward kernels
 constexpr int kThreadsBwd = 256;       // backward and Sinkhorn kernels
 static_assert(kThreads == kSmStride, "the scratch column stride is the block size");
 
-// largest in-row logit range max_i (max_j H_ij - min_j H_ij) up to which a matrix starts from beta = 0 (above: LP
-// dual start); chosen by measurement, S1.  Row offsets do not matter: eq. (10) removes them.
-constexpr float kLpRange = 12.0f;
 #ifdef BK4_EXPERIMENTS
 static float lp_range_exp() { const char* e = getenv("BK4_LPRANGE"); return e ? (float)atof(e) : kLpRange; }
 #endif
@@ -93,98 +90,45 @@ __global__ void __launch_bounds__(kThreads, 1024 / kThreads) forward_kernel(cons
             store_matrix(bwd.dH + 16 * idx, d);
         }
     };
-    bool left = valid;  // this thread's matrix still has to be solved
-    int it_lean = 0;    // updates the lean iteration spent on it
-    if constexpr (!GUARDED_ONLY) {
-        float h[16];
-        load_logits<BF16>(H, idx, h);
-        // row maxima (the shift of eq. (10)) and the largest in-row range, which decides the start.
-        // A NaN logit is skipped by fmaxf/fminf: such a matrix fails the first residual test and ends up in the
-        // guarded solver, which reports it; an infinite logit makes the range infinite and is sent there at once.
-        float rmax[4], spread = 0.0f;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            rmax[i] = fmaxf(fmaxf(h[4 * i], h[4 * i + 1]), fmaxf(h[4 * i + 2], h[4 * i + 3]));
-            const float rmin = fminf(fminf(h[4 * i], h[4 * i + 1]), fminf(h[4 * i + 2], h[4 * i + 3]));
-            spread = fmaxf(spread, rmax[i] - rmin);
-        }
-        const bool finite = valid && spread <= 3.0e38f;  // an infinite (or inf - inf = NaN) range is the guarded solver's
-        bool narrow = finite && spread <= lp_range;
-        float E[16], T[16], v0, v1, v2;
-        if (__any_sync(0xffffffffu, narrow)) {
-            float s0[4];
-            const float smax = narrow_exponentials(h, rmax, E, s0);
-            narrow = narrow && !(smax < kPeakedSum);
-            if (__any_sync(0xffffffffu, narrow)) narrow_sweeps(E, s0, v0, v1, v2);
-        }
-        const bool wide = finite && !narrow, active = finite;
-        const bool any_narrow = __any_sync(0xffffffffu, narrow), any_wide = __any_sync(0xffffffffu, wide);
-        if (any_narrow || any_wide) {
-            LeanResult res;
-            if (any_wide) {
-                // the wide start works on column-permuted matrices: a narrow matrix in the same warp keeps its order
-                float Ew[16], w0, w1, w2;
-                unsigned code;
-                wide_start(h, sm, Ew, w0, w1, w2, code);
-                if (wide || !any_narrow) {
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) E[q] = Ew[q];
-                    v0 = w0, v1 = w1, v2 = w2;
-                } else {
-                    code = kIdentityCode;
-                }
-                res = lean_iterate(E, v0, v1, v2, active, tol_i, max_iter, T);
-                if (active && res.stored) {
-                    float out[16];
-                    unpermute_columns(T, code, sm, out);
-                    commit(out);
-                }
-            } else {
-                res = lean_iterate(E, v0, v1, v2, active, tol_i, max_iter, T);
-                if (active && res.stored) commit(T);
-            }
-            if (active && res.stored) record(res.it, res.converged);
-            left = valid && !(active && res.stored);
-            it_lean = active ? res.it : 0;
-        }
-    }
-    if (__any_sync(0xffffffffu, left)) {
-        if (left) {  // every lane for itself: this is the rare path
-            float h[16];
-            load_logits<BF16>(H, idx, h);  // the lean part has stored only matrices this branch does not touch
-            float poison = 0.0f;
-#pragma unroll
-            for (int q = 0; q < 16; ++q) poison = __fmaf_rn(h[q], 0.0f, poison);  // NaN iff some logit is NaN or +-Inf
-            const bool bad = !(poison == 0.0f);
-            // LP dual potentials and the column permutation (a NaN/Inf matrix goes through the motions and is
-            // overwritten with NaN)
-            float w[4][4], xs[4], hc[16];
-            unsigned code;
-            lp_dual(h, sm, w, xs, code);
-            gather_columns(sm, code, hc);
-            auto gather = [&](float(&Hr)[16]) {
-                float hr[16];
-                load_logits<BF16>(H, idx, hr);
-#pragma unroll
-                for (int q = 0; q < 16; ++q) sm[q * kSmStride] = hr[q];
-                gather_columns(sm, code, Hr);
-            };
-            auto emit = [&](const float(&T)[16], int iters, bool converged) {
-                float out[16];
-                unpermute_columns(T, code, sm, out);
-#pragma unroll
-                for (int q = 0; q < 16; ++q) out[q] = bad ? kNaN : out[q];
-                commit(out);
-                record(it_lean + iters, converged && !bad);
-            };
-            newton_guarded(hc, xs, tol_i, max_iter > it_lean ? max_iter - it_lean : 0, gather, emit);
-        }
-    }
+    auto load = [&](float(&h)[16]) { load_logits<BF16>(H, idx, h); };
+    project_one<GUARDED_ONLY>(load, valid, sm, tol_i, max_iter, lp_range, commit, record);
     if constexpr (DIAG) {
         __syncthreads();
         if (diag.hist && threadIdx.x < BIRKHOFF4_HIST_BINS && s_hist[threadIdx.x])
             atomicAdd(&diag.hist[threadIdx.x], (unsigned long long)s_hist[threadIdx.x]);
         if (diag.n_unconverged && threadIdx.x == 0 && s_unc) atomicAdd(diag.n_unconverged, (unsigned long long)s_unc);
+    }
+}
+
+// ---------------------------------------------------------------- fused consumer: projection + residual-stream mix
+template <bool XBF16>
+__global__ void __launch_bounds__(kThreads, 512 / kThreads) forward_mix_kernel(
+    const float* __restrict__ H, const typename MixVec<XBF16>::elem* __restrict__ X, typename MixVec<XBF16>::elem* __restrict__ Y,
+    float* __restrict__ P, int64_t B, int C, float tol_i, int max_iter, float lp_range) {
+    pdl_wait_and_trigger();
+    __shared__ float s_col[16 * kThreads];
+    float* const sm = s_col + threadIdx.x;
+    const int64_t tok0 = (int64_t)blockIdx.x * kMixTokens;
+    const int64_t b = tok0 + threadIdx.x;
+    const bool valid = b < B;
+    const int64_t idx = valid ? b : B - 1;
+    // phase 1: thread t projects token t; the result stays in the thread's shared-memory column
+    auto load = [&](float(&h)[16]) { load_matrix(H + 16 * idx, h); };
+    auto commit = [&](const float(&out)[16]) {
+        if (P) store_matrix(P + 16 * idx, out);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) sm[q * kSmStride] = out[q];
+    };
+    auto record = [](int, bool) {};
+    project_one<false>(load, valid, sm, tol_i, max_iter, lp_range, commit, record);
+    __syncthreads();
+    // phase 2: the block streams its tokens' 4 x C activations
+    const int ntok = (int)((B - tok0 < kMixTokens) ? B - tok0 : kMixTokens);
+    for (int t = 0; t < ntok; ++t) {
+        float p[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) p[q] = s_col[q * kSmStride + t];  // the same address for every thread: a broadcast
+        mix_token<XBF16>(p, X + (size_t)(tok0 + t) * 4 * C, Y + (size_t)(tok0 + t) * 4 * C, C);
     }
 }
 
@@ -344,6 +288,19 @@ static int run_host(const float* H_host, const float* P_in_host, const float* dP
     return rc;
 }
 
+template <bool XBF16>
+static int launch_mix(const float* H, const void* X, void* Y, float* P, int64_t B, int C, float tol, int max_iter,
+                      cudaStream_t stream) {
+    using E = typename MixVec<XBF16>::elem;
+    if (B < 0 || !(tol >= 0.0f) || max_iter < 0 || C < 1 || C % MixVec<XBF16>::kElems) return BIRKHOFF4_EINVAL;
+    if (B == 0) return BIRKHOFF4_OK;
+    if (!H || !X || !Y || misaligned(H) || misaligned(P) || (reinterpret_cast<uintptr_t>(X) & 15u) ||
+        (reinterpret_cast<uintptr_t>(Y) & 15u))
+        return BIRKHOFF4_EINVAL;
+    return cuda_rc(launch(forward_mix_kernel<XBF16>, grid_for(B, kMixTokens), kThreads, stream, H, (const E*)X, (E*)Y, P, B, C,
+                          internal_tol(tol), max_iter, kLpRange));
+}
+
 }  // namespace bk4
 
 // =================================================================== C ABI
@@ -379,6 +336,16 @@ int birkhoff4_forward_backward(const float* H, const float* dP, float* P, float*
                                birkhoff4_stream_t stream) {
     return launch_forward<false, false, true>(H, P, B, tol, max_iter, FwdDiag{nullptr, nullptr, nullptr}, (cudaStream_t)stream,
                                               FusedBwd{dP, dH});
+}
+
+int birkhoff4_forward_mix(const float* H, const float* X, float* Y, float* P, int64_t B, int C, float tol, int max_iter,
+                          birkhoff4_stream_t stream) {
+    return launch_mix<false>(H, X, Y, P, B, C, tol, max_iter, (cudaStream_t)stream);
+}
+
+int birkhoff4_forward_mix_bf16(const float* H, const uint16_t* X, uint16_t* Y, float* P, int64_t B, int C, float tol,
+                               int max_iter, birkhoff4_stream_t stream) {
+    return launch_mix<true>(H, X, Y, P, B, C, tol, max_iter, (cudaStream_t)stream);
 }
 
 int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, birkhoff4_stream_t stream) {

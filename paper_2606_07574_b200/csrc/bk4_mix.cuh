@@ -1,0 +1,75 @@
+// bk4_mix.cuh -- the fused consumer of the projection: the residual-stream mix
+// x_{l+1} = H^res x_l of PAPER.md:46-50 with H^res = proj(exp(H)) computed in the same kernel, so that the
+// doubly-stochastic matrix never makes the round trip through HBM that the separate calls pay (64 B written + 64 B
+// re-read per token; the mix itself is bound by the 4 C elements of x_l in and out).
+//
+// One block = kMixTokens tokens.  Phase 1: thread t projects token t's matrix (project_one: the same code as
+// birkhoff4_forward) and leaves P_t in its shared-memory column.  Phase 2: the block streams the tokens' 4 x C
+// activations: every thread reads P_t (a broadcast) and mixes a 16-byte slice of each of the four streams.
+#pragma once
+#include <cuda_bf16.h>
+
+#include "bk4_project.cuh"
+
+namespace bk4 {
+
+constexpr int kMixTokens = BK4_THREADS;  // tokens per block = threads per block (one matrix per thread in phase 1)
+
+template <bool XBF16>
+struct MixVec;
+template <>
+struct MixVec<false> {  // fp32 activations: 4 elements per 16-byte access
+    static constexpr int kElems = 4;
+    using elem = float;
+    BK4_DEV static void load(const float* p, float (&x)[4]) {
+        const float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+        x[0] = t.x, x[1] = t.y, x[2] = t.z, x[3] = t.w;
+    }
+    BK4_DEV static void store(float* p, const float (&y)[4]) {
+        __stcs(reinterpret_cast<float4*>(p), make_float4(y[0], y[1], y[2], y[3]));
+    }
+};
+template <>
+struct MixVec<true> {  // bf16 activations (bit patterns): 8 elements per 16-byte access, fp32 accumulation
+    static constexpr int kElems = 8;
+    using elem = uint16_t;
+    BK4_DEV static void load(const uint16_t* p, float (&x)[8]) {
+        const uint4 t = __ldcs(reinterpret_cast<const uint4*>(p));
+        const uint32_t w[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            x[2 * k] = __uint_as_float(w[k] << 16);
+            x[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+        }
+    }
+    BK4_DEV static void store(uint16_t* p, const float (&y)[8]) {
+        uint32_t w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const __nv_bfloat162 h = __floats2bfloat162_rn(y[2 * k], y[2 * k + 1]);  // round to nearest even
+            w[k] = *reinterpret_cast<const uint32_t*>(&h);
+        }
+        __stcs(reinterpret_cast<uint4*>(p), make_uint4(w[0], w[1], w[2], w[3]));
+    }
+};
+
+// phase 2 for one token: y_i = sum_j P_ij x_j over this thread's slices of the C columns
+template <bool XBF16>
+BK4_DEV void mix_token(const float (&p)[16], const typename MixVec<XBF16>::elem* x, typename MixVec<XBF16>::elem* y, int C) {
+    constexpr int V = MixVec<XBF16>::kElems;
+    for (int c = threadIdx.x * V; c < C; c += kMixTokens * V) {
+        float xin[4][V], yout[V];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) MixVec<XBF16>::load(x + (size_t)j * C + c, xin[j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+#pragma unroll
+            for (int e = 0; e < V; ++e)
+                yout[e] = fmaf(p[4 * i + 3], xin[3][e],
+                               fmaf(p[4 * i + 2], xin[2][e], fmaf(p[4 * i + 1], xin[1][e], p[4 * i] * xin[0][e])));
+            MixVec<XBF16>::store(y + (size_t)i * C + c, yout);
+        }
+    }
+}
+
+}  // namespace bk4

@@ -641,3 +641,50 @@ def test_fused_forward_backward_mixed_and_nonfinite():
     assert L.birkhoff4_forward_backward(p, None, p, p, 4, 1e-6, 20, None) == 1       # dP missing
     assert L.birkhoff4_forward_backward(p, p, None, None, 4, 1e-6, 20, None) == 1    # dH missing
     assert L.birkhoff4_forward_backward(None, None, None, None, 0, 1e-6, 20, None) == 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# fused consumer: Y_b = proj(exp(H_b)) X_b in one kernel.  The oracle is the
+# definition: the fp64 oracle's P times X (a matrix product, numpy).
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("B,C", [(1, 8), (129, 64), (1000, 1024), (4097, 200)])
+def test_fused_mix_matches_oracle(oracle, B, C, dtype):
+    H = inputs.normal(B, 3.0, config=98, sub=B)[0]
+    X = np.random.Generator(np.random.Philox(key=inputs.SEED + 99 + B)).standard_normal((B, 4, C), dtype=np.float32)
+    Hd = dev(H)
+    if dtype == "bf16":
+        Xb = inputs.f32_to_bf16_bits(X)
+        X = inputs.bf16_bits_to_f32(Xb)                                 # the oracle sees what the kernel sees
+        Xd = torch.from_numpy(Xb.view(np.int16)).cuda().view(torch.bfloat16)
+    else:
+        Xd = dev(X)
+    ybuf = torch.full((B + 2, 4, C), 7.0, device="cuda", dtype=Xd.dtype)
+    Y, P = bk.birkhoff4_forward_mix(Hd, Xd, ybuf[1:B + 1], want_P=True, max_iter=32)
+    assert (ybuf[0].float() == 7.0).all() and (ybuf[B + 1].float() == 7.0).all()   # guard cells
+    assert torch.equal(P, bk.birkhoff4_forward(Hd, max_iter=32))        # the same projection, bit for bit
+    P_o = oracle.forward(H.astype(np.float64))
+    Y_o = np.einsum("bij,bjc->bic", P_o, X.astype(np.float64))
+    Yh = host(Y.float()).astype(np.float64)
+    tol = 2.0 ** -8 if dtype == "bf16" else 2e-6                        # bf16: half an ulp of the stored result
+    assert (np.abs(Yh - Y_o) <= tol * np.maximum(np.abs(Y_o), 1.0) + 1e-6).all()
+    Y2, none = bk.birkhoff4_forward_mix(Hd, Xd, max_iter=32)            # P not requested: never written
+    assert none is None and torch.equal(Y2, Y)
+
+
+def test_fused_mix_edges():
+    H = dev(inputs.normal(64, 1.0, config=98)[0])
+    X = torch.zeros((64, 4, 16), device="cuda")
+    L = bk.lib()
+    import ctypes
+    ph, px = ctypes.c_void_p(H.data_ptr()), ctypes.c_void_p(X.data_ptr())
+    assert L.birkhoff4_forward_mix(ph, px, px, None, 64, 6, 1e-6, 20, None) == 1      # C not a multiple of 4
+    assert L.birkhoff4_forward_mix(ph, None, px, None, 64, 16, 1e-6, 20, None) == 1
+    assert L.birkhoff4_forward_mix(ph, ctypes.c_void_p(X.data_ptr() + 4), px, None, 64, 16, 1e-6, 20, None) == 1
+    assert L.birkhoff4_forward_mix(None, None, None, None, 0, 16, 1e-6, 20, None) == 0
+    with pytest.raises(bk.Birkhoff4Error):
+        bk.birkhoff4_forward_mix(H, torch.zeros((63, 4, 16), device="cuda"))
+    Hn = H.clone()
+    Hn[3, 0, 0] = float("nan")
+    Y, _ = bk.birkhoff4_forward_mix(Hn, torch.ones((64, 4, 16), device="cuda"))
+    assert bool(torch.isnan(Y[3]).all()) and bool(torch.isfinite(Y[4]).all())
+    assert (Y[4].sum(0) - 4.0).abs().max().item() < 1e-5               # columns of P sum to 1: the mix conserves the stream sum
