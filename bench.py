@@ -138,19 +138,6 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(kernel, B):
-    """dram bytes per launch of `kernel` at batch B from the committed ncu --set full summary, or None"""
-    p = os.path.join(ROOT, "profiles", "traffic.csv")
-    if not os.path.exists(p):
-        return None
-    with open(p) as f:
-        for line in f:
-            k = [x.strip() for x in line.split(",")]
-            if len(k) >= 4 and k[0] == kernel and k[1] == str(B):
-                return float(k[2]) + float(k[3])
-    return None
-
-
 def _finite(x):
     """strict JSON: NaN/Inf (e.g. the Sinkhorn-20 baseline's error at s >= 30, where exp underflows) become null"""
     if isinstance(x, float):
@@ -199,6 +186,206 @@ def run_reference(args, wl):
 
 
 # ------------------------------------------------------------------------------------------------ our arm
+def _rooflines(B, bf16, f_us, b_us, s_us, peak, peak_src, workload, mean_updates, sm_mhz, n_sm):
+    """per-kernel and per-step achieved HBM bandwidth against the measured copy peak, and the forward's second
+    roofline (instruction issue, from the ncu instruction count of this workload under profiles/)"""
+    fb = 96 if bf16 else FWD_BYTES
+    nominal = 7700.0                                                           # B200_PROFILING.md: HGX nominal HBM3e GB/s
+    k = {}
+    for name, us, byts in (("forward_kernel", f_us, fb), ("backward_kernel", b_us, BWD_BYTES)):
+        ach = B * byts / (us["median"] * 1e-6) / 1e9
+        k[name] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                   "frac_min_time": B * byts / (us["min"] * 1e-6) / 1e9 / peak, "frac_of_nominal_7700": ach / nominal,
+                   "avg_us": us["median"], "min_us": us["min"], "bytes_per_launch": B * byts,
+                   "traffic": ncu_traffic(name, workload)}
+        if k[name]["frac"] > 1.0:
+            k[name]["note"] = "above 1: the measured copy peak underestimates what a pure stream reaches"
+    ach = B * (fb + BWD_BYTES) / (s_us["median"] * 1e-6) / 1e9
+    step = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "bytes_per_step": B * (fb + BWD_BYTES),
+            "peak_source": peak_src}
+    winst = ncu_warp_inst("forward_kernel", workload)
+    if winst:
+        issue_peak = 4.0 * n_sm * sm_mhz * 1e6                                 # warp instructions / s
+        ach_i = winst * (B / 32.0) / (f_us["median"] * 1e-6)
+        k["forward_kernel"]["alu"] = {
+            "bound": "alu", "achieved": ach_i / 1e12, "peak": issue_peak / 1e12, "unit": "T warp-instr/s", "frac": ach_i / issue_peak,
+            "warp_instr_per_32_matrices": winst, "source": "ncu smsp__inst_executed.sum of this workload (profiles/traffic.csv)",
+            "peak_source": "nominal: 4 issue slots per clock per SM x %d SMs x %d MHz (half-rate instructions hold a slot for "
+                           "two clocks, profiles/r2_pipe_microbench.md: the attainable fraction is below 1)" % (n_sm, sm_mhz)}
+    return k, step
+
+
+def ncu_warp_inst(kernel, workload):
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            k = [x.strip() for x in line.split(",")]
+            if len(k) >= 5 and k[0] == kernel and k[1] == workload:
+                return float(k[4])
+    return None
+
+
+def ncu_traffic(kernel, workload):
+    """dram bytes per launch of `kernel` on `workload` from the committed ncu --set full summaries, or None"""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            k = [x.strip() for x in line.split(",")]
+            if len(k) >= 4 and k[0] == kernel and k[1] == workload:
+                return float(k[2]) + float(k[3])
+    return None
+
+
+class Timer:
+    """R timed regions of K calls each, CUDA events on the launching (current) stream; per-call us: median and min"""
+
+    def __init__(self, torch, K, R):
+        self.torch, self.K, self.R = torch, K, R
+
+    def __call__(self, fn):
+        t = self.torch
+        per = []
+        for _ in range(self.R):
+            e0, e1 = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(self.K):
+                fn(i)
+            e1.record()
+            e1.synchronize()
+            per.append(e0.elapsed_time(e1) * 1e3 / self.K)
+        return {"median": statistics.median(per), "min": min(per), "regions": self.R, "calls_per_region": self.K}
+
+
+def err_stats(torch, P):
+    """Err of PAPER.md:323 in fp64 on the stored fp32 P: max, mean, and the largest single marginal deviation"""
+    mx, sm, einf, n = 0.0, 0.0, 0.0, P.shape[0]
+    for lo in range(0, n, 1 << 22):
+        P64 = P[lo:lo + (1 << 22)].double()
+        r, c = (P64.sum(2) - 1).abs(), (P64.sum(1) - 1).abs()
+        e = r.sum(1) + c.sum(1)
+        mx, sm = max(mx, float(e.max())), sm + float(e.sum())
+        einf = max(einf, float(r.max()), float(c.max()))
+        del P64, r, c, e
+    return {"max_marginal_err": mx, "mean_marginal_err": sm / n, "max_err_inf": einf}
+
+
+def measure_workload(torch, bk, inputs, name, wl, rank, K, R, peak, peak_src, sm_mhz, n_sm, max_iter=None, sort_by_class=False):
+    """device-resident measurement of one workload: forward, backward and step timings, accuracy, histogram"""
+    B, bf16 = wl["B"], wl["config"] == 4
+    max_iter = wl["max_iter"] if max_iter is None else max_iter
+    set_bytes = B * (32 if bf16 else 64) + 3 * B * 64
+    nsets = max(2, -(-(1 << 30) // set_bytes))                                 # >= 1 GiB in rotation (L2 is 126 MB)
+    distinct = 1 if B > (1 << 21) else nsets                                   # large B: one draw, copied (host time)
+    sets = []
+    for k in range(nsets):
+        if k < distinct:
+            if wl["config"] == 5:
+                H, G, _ = inputs.heterogeneous(B, config=5, sub=100 * rank + k, sort_by_class=sort_by_class)
+            else:
+                H, G = make_inputs(wl, rank, k)
+            H0, G0 = (H, G) if k == 0 else (H0, G0)
+        Hd = torch.from_numpy(H.view(np.int16)).cuda().view(torch.bfloat16) if bf16 else torch.from_numpy(H).cuda()
+        sets.append(dict(H=Hd, G=torch.from_numpy(G).cuda(), P=torch.empty((B, 4, 4), device="cuda"),
+                         dH=torch.empty((B, 4, 4), device="cuda")))
+    fwd = bk.birkhoff4_forward_bf16 if bf16 else bk.birkhoff4_forward
+
+    def f_call(i):
+        s = sets[i % nsets]
+        fwd(s["H"], s["P"], TOL, max_iter)
+
+    def b_call(i):
+        t = sets[i % nsets]
+        bk.birkhoff4_backward(t["P"], t["G"], t["dH"])
+
+    def step(i):
+        s, t = sets[i % nsets], sets[(i + 1) % nsets]
+        fwd(s["H"], s["P"], TOL, max_iter)
+        bk.birkhoff4_backward(t["P"], t["G"], t["dH"])
+
+    for i in range(nsets):                                                     # every set has a valid P before backward reads it
+        f_call(i)
+    for i in range(3):
+        step(i)
+    torch.cuda.synchronize()
+    timer = Timer(torch, K, R)
+    s_us, f_us, b_us = timer(step), timer(f_call), timer(b_call)
+    acc = err_stats(torch, sets[0]["P"])
+    hist = torch.zeros(64, dtype=torch.int64, device="cuda")
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    (bk.birkhoff4_forward_bf16_ex if bf16 else bk.birkhoff4_forward_ex)(sets[0]["H"], sets[0]["P"], TOL, max_iter,
+                                                                        hist=hist, n_unconverged=unc)
+    h = hist.cpu().numpy()
+    mean_updates = float((h * np.arange(64)).sum() / max(h.sum(), 1))
+    kern, step_roof = _rooflines(B, bf16, f_us, b_us, s_us, peak, peak_src, name, mean_updates, sm_mhz, n_sm)
+    res = {"desc": wl["desc"] + (", sorted by class" if sort_by_class else ""), "B": B, "max_iter": max_iter,
+           "value": B / (s_us["median"] * 1e-6), "unit": UNIT, "step_us": s_us, "forward_us": f_us, "backward_us": b_us,
+           "fwd_matrices_per_s": B / (f_us["median"] * 1e-6), "roofline_step": step_roof, "roofline_kernels": kern,
+           "mean_newton_updates": mean_updates,
+           "update_histogram": {str(k): round(float(h[k]) / max(h.sum(), 1), 6) for k in range(64) if h[k]},
+           "unconverged": int(unc.item()), "buffer_sets": nsets, **acc}
+    return res, sets, (H0, G0)
+
+
+def measure_widenings(torch, bk, inputs, K, R, peak):
+    """fused forward+backward, n = 8, general OT, fused mix: per-call us and achieved HBM GB/s"""
+    timer = Timer(torch, K, R)
+    out = {}
+    B = 1 << 20
+    H, G = inputs.normal(B, 1.0, config=2)
+    sets = [dict(H=torch.from_numpy(H).cuda() + 0 * k, G=torch.from_numpy(G).cuda(), P=torch.empty((B, 4, 4), device="cuda"),
+                 dH=torch.empty((B, 4, 4), device="cuda")) for k in range(4)]
+    for want_P, byts in ((True, 256), (False, 192)):
+        us = timer(lambda i: bk.birkhoff4_forward_backward(sets[i % 4]["H"], sets[i % 4]["G"], sets[i % 4]["P"] if want_P else None,
+                                                           sets[i % 4]["dH"], TOL, 20, want_P=want_P))
+        out["fused_forward_backward" + ("" if want_P else "_no_P")] = {
+            "desc": "B=2^20 N(0,1), one kernel, P %s" % ("written" if want_P else "not written"), "us": us,
+            "bytes_per_matrix": byts, "achieved_GBs": B * byts / (us["median"] * 1e-6) / 1e9,
+            "frac": B * byts / (us["median"] * 1e-6) / 1e9 / peak, "matrices_per_s": B / (us["median"] * 1e-6)}
+    del sets
+    B8 = 1 << 18
+    for s in (1.0, 10.0):
+        H8, G8 = inputs.normal_n(B8, 8, s, config=8)
+        s8 = [dict(H=torch.from_numpy(H8).cuda() + 0 * k, G=torch.from_numpy(G8).cuda(), P=torch.empty((B8, 8, 8), device="cuda"),
+                   dH=torch.empty((B8, 8, 8), device="cuda")) for k in range(4)]
+        fus = timer(lambda i: bk.birkhoff8_forward(s8[i % 4]["H"], s8[i % 4]["P"], 2e-6, 60))
+        bus = timer(lambda i: bk.birkhoff8_backward(s8[i % 4]["P"], s8[i % 4]["G"], s8[i % 4]["dH"]))
+        P64 = s8[0]["P"].double()
+        err = float(((P64.sum(2) - 1).abs().sum(1) + (P64.sum(1) - 1).abs().sum(1)).max())
+        out["birkhoff8_s%g" % s] = {
+            "desc": "B=2^18 fp32 8x8, H iid N(0,%g^2)" % s, "forward_us": fus, "backward_us": bus, "max_marginal_err": err,
+            "forward": {"bytes_per_matrix": 512, "frac": B8 * 512 / (fus["median"] * 1e-6) / 1e9 / peak,
+                        "matrices_per_s": B8 / (fus["median"] * 1e-6)},
+            "backward": {"bytes_per_matrix": 768, "frac": B8 * 768 / (bus["median"] * 1e-6) / 1e9 / peak,
+                         "matrices_per_s": B8 / (bus["median"] * 1e-6)}}
+        del s8, P64
+    Bo = 1 << 20
+    Cm, a, b, Go = inputs.ot_problem(Bo, 4, 4, 2.0, config=9)
+    so = [dict(C=torch.from_numpy(Cm).cuda() + 0 * k, a=torch.from_numpy(a).cuda(), b=torch.from_numpy(b).cuda(),
+               G=torch.from_numpy(Go).cuda(), T=torch.empty((Bo, 4, 4), device="cuda"), D=torch.empty((Bo, 4, 4), device="cuda"))
+          for k in range(4)]
+    fus = timer(lambda i: bk.entropic_ot_forward(so[i % 4]["C"], so[i % 4]["a"], so[i % 4]["b"], so[i % 4]["T"], 0.7, 2e-6, 60))
+    bus = timer(lambda i: bk.entropic_ot_backward(so[i % 4]["T"], so[i % 4]["G"], so[i % 4]["D"], 0.7))
+    out["entropic_ot_4x4"] = {"desc": "B=2^20 4x4 costs N(0,2^2), Gamma(4) marginals, eta = 0.7", "forward_us": fus, "backward_us": bus,
+                              "forward": {"bytes_per_matrix": 160, "frac": Bo * 160 / (fus["median"] * 1e-6) / 1e9 / peak},
+                              "backward": {"bytes_per_matrix": 192, "frac": Bo * 192 / (bus["median"] * 1e-6) / 1e9 / peak}}
+    del so
+    Bm, C = 1 << 16, 1024
+    Hm = torch.from_numpy(inputs.normal(Bm, 1.0, config=2, sub=7)[0]).cuda()
+    g = torch.Generator(device="cuda").manual_seed(inputs.SEED + 77)
+    Xs = [torch.randn((Bm, 4, C), device="cuda", generator=g).bfloat16() for _ in range(2)]
+    Ys = [torch.empty_like(x) for x in Xs]
+    us = timer(lambda i: bk.birkhoff4_forward_mix(Hm, Xs[i % 2], Ys[i % 2], None, TOL, 20))
+    byts = 64 + 2 * 4 * C * 2
+    out["fused_mix_bf16"] = {"desc": "B=2^16 tokens, 4 streams x C=1024 bf16: Y = proj(exp(H)) X in one kernel", "us": us,
+                             "bytes_per_token": byts, "achieved_GBs": Bm * byts / (us["median"] * 1e-6) / 1e9,
+                             "frac": Bm * byts / (us["median"] * 1e-6) / 1e9 / peak, "tokens_per_s": Bm / (us["median"] * 1e-6)}
+    return out
+
+
 def run_ours(args, wl):
     import torch
     import torch.distributed as dist
@@ -212,27 +399,10 @@ def run_ours(args, wl):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     bk.lib()                                                                   # raises if libbirkhoff4.so cannot be had
-    if args.variant:
-        bk.birkhoff4_set_variant(args.variant)                                 # measurement only; 0 = library default
-
+    props = torch.cuda.get_device_properties(local)
+    peak, peak_src = measured_peaks()
     B, bf16, max_iter = wl["B"], wl["config"] == 4, wl["max_iter"]
-    set_bytes = B * (32 if bf16 else 64) + 3 * B * 64
-    nsets = max(2, -(-(1 << 30) // set_bytes))                                 # >= 1 GiB in rotation
-    sets = []
-    distinct = 1 if B > (1 << 22) else nsets                                   # 2^24: one draw, copied (host RAM/time)
-    for k in range(nsets):
-        if k < distinct:
-            H, G = make_inputs(wl, rank, k)
-            H0, G0 = H, G
-        Hd = torch.from_numpy(H.view(np.int16)).cuda().view(torch.bfloat16) if bf16 else torch.from_numpy(H).cuda()
-        sets.append(dict(H=Hd, G=torch.from_numpy(G).cuda(), P=torch.empty((B, 4, 4), device="cuda"),
-                         dH=torch.empty((B, 4, 4), device="cuda")))
-    fwd = bk.birkhoff4_forward_bf16 if bf16 else bk.birkhoff4_forward
-
-    def step(i):
-        s, t = sets[i % nsets], sets[(i + 1) % nsets]
-        fwd(s["H"], s["P"], TOL, max_iter)
-        bk.birkhoff4_backward(t["P"], t["G"], t["dH"])
+    K, R = args.steps, args.regions
 
     def barrier():
         torch.cuda.synchronize()
@@ -240,83 +410,50 @@ def run_ours(args, wl):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for s in sets:                                                             # every set has a valid P before backward reads it
-        fwd(s["H"], s["P"], TOL, max_iter)
-    for i in range(max(args.warmup, 3)):
-        step(i)
     clocks = ClockSampler(local)
     clocks.start()
+    sm_mhz = clocks.max_mhz or 1965
 
-    # ---- device-timed region: K steps, events on the launching (current) stream
-    K = args.steps
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
-    barrier()
+    # ---- warm-up + the contract's timed region: EXACTLY K steps between two events, barrier + synchronize on both sides
+    head, sets, (H0, G0) = None, None, (None, None)
     clocks.region(True)
+    head, sets, (H0, G0) = measure_workload(torch, bk, inputs, args.workload, wl, rank, K, R, peak, peak_src, sm_mhz,
+                                            props.multi_processor_count)
+    nsets = len(sets)
+    fwd = bk.birkhoff4_forward_bf16 if bf16 else bk.birkhoff4_forward
+
+    def step(i):
+        s, t = sets[i % nsets], sets[(i + 1) % nsets]
+        fwd(s["H"], s["P"], TOL, max_iter)
+        bk.birkhoff4_backward(t["P"], t["G"], t["dH"])
+
+    for i in range(max(args.warmup, 3)):
+        step(i)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    barrier()
     ev[0].record()
     for i in range(K):
         step(i)
     ev[1].record()
     clocks.sample()
     barrier()
-    total_ms = ev[0].elapsed_time(ev[1])
-    # per-kernel average launch duration, same region, same rotation: K launches of one kernel between two events
-    ev[2].record()
-    for i in range(K):
-        s = sets[i % nsets]
-        fwd(s["H"], s["P"], TOL, max_iter)
-    ev[3].record()
-    barrier()
-    ev[4].record()
-    for i in range(K):
-        t = sets[i % nsets]
-        bk.birkhoff4_backward(t["P"], t["G"], t["dH"])
-    ev[5].record()
-    barrier()
-    clocks.region(False)
-    f_ms, b_ms = ev[2].elapsed_time(ev[3]) / K, ev[4].elapsed_time(ev[5]) / K
-    total_ms = shard.reduce_max_time(total_ms, dist if world > 1 else None)
+    total_ms = shard.reduce_max_time(ev[0].elapsed_time(ev[1]), dist if world > 1 else None)
     value = world * B * K / (total_ms * 1e-3)
-
-    # ---- accuracy of what was just computed (set 0), PAPER.md:323 in fp64
-    P64 = sets[0]["P"].double()
-    err = ((P64.sum(2) - 1).abs().sum(1) + (P64.sum(1) - 1).abs().sum(1))
-    max_err, mean_err = float(err.max()), float(err.mean())
-    hist = torch.zeros(64, dtype=torch.int64, device="cuda")
-    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
-    (bk.birkhoff4_forward_bf16_ex if bf16 else bk.birkhoff4_forward_ex)(sets[0]["H"], sets[0]["P"], TOL, max_iter,
-                                                                        hist=hist, n_unconverged=unc)
-    h = hist.cpu().numpy()
-    mean_updates = float((h * np.arange(64)).sum() / max(h.sum(), 1))
-    update_hist = {str(k): round(float(h[k]) / max(h.sum(), 1), 6) for k in range(64) if h[k]}
-    del P64, err
 
     # ---- Sinkhorn-20 baseline kernel of the same library (context: PAPER.md:32, 319), fp32 workloads only
     sink = None
     if not bf16:
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        n_s = min(K, 200)
-        torch.cuda.synchronize()
-        e0.record()
-        for i in range(n_s):
-            s = sets[i % nsets]
-            bk.birkhoff4_sinkhorn(s["H"], s["dH"], 20)
-        e1.record()
-        torch.cuda.synchronize()
-        T64 = sets[(n_s - 1) % nsets]["dH"].double()
-        serr = ((T64.sum(2) - 1).abs().sum(1) + (T64.sum(1) - 1).abs().sum(1))
-        sink = {"fwd_matrices_per_s": B * n_s / (e0.elapsed_time(e1) * 1e-3), "max_marginal_err": float(serr.max()),
-                "mean_marginal_err": float(serr.mean())}
-        del T64, serr
+        us = Timer(torch, min(K, 50), 3)(lambda i: bk.birkhoff4_sinkhorn(sets[i % nsets]["H"], sets[i % nsets]["dH"], 20))
+        sink = {"fwd_matrices_per_s": B / (us["median"] * 1e-6), "us": us, **err_stats(torch, sets[0]["dH"])}
 
     # ---- end to end: pinned host buffers through the host-buffer C-ABI call, copies inside the timed region
     Hh = torch.from_numpy(inputs.bf16_bits_to_f32(H0) if bf16 else H0).pin_memory()
     Gh = torch.from_numpy(G0).pin_memory()
     Ph, dHh = torch.empty_like(Hh).pin_memory(), torch.empty_like(Hh).pin_memory()
-    K_e = K if B * K <= (1 << 28) else max(3, (1 << 28) // B)                  # bounded: <= 2^28 matrices end to end
+    K_e = K if B * K <= (1 << 27) else max(3, (1 << 27) // B)                  # bounded: <= 2^27 matrices end to end
     for _ in range(2):
         bk.birkhoff4_forward_backward_host(Hh, Gh, Ph, dHh, TOL, max_iter)
     barrier()
-    clocks.region(True)
     t0 = time.perf_counter()
     for _ in range(K_e):
         bk.birkhoff4_forward_backward_host(Hh, Gh, Ph, dHh, TOL, max_iter)     # synchronous: outputs are in host memory
@@ -328,51 +465,57 @@ def run_ours(args, wl):
            "d2h_bytes_per_step": 2 * B * 64, "steps": K_e,
            "api": "birkhoff4_forward_backward_host(H_host, dP_host -> P_host, dH_host), fp32 pinned host buffers"}
     bk.birkhoff4_host_release()
-    clocks.stop()
+    del sets, Hh, Gh, Ph, dHh
+    torch.cuda.empty_cache()
 
+    launches = 2 * K
     if rank != 0:
+        clocks.stop()
         if world > 1:
             dist.destroy_process_group()
         return
-    peak, peak_src = measured_peaks()
-    fb = 96 if bf16 else FWD_BYTES
-    kernels = {
-        "forward_lean_kernel": {"bound": "hbm", "achieved": B * fb / (f_ms * 1e-3) / 1e9, "avg_us": f_ms * 1e3,
-                           "bytes_per_launch": B * fb},
-        "backward_kernel": {"bound": "hbm", "achieved": B * BWD_BYTES / (b_ms * 1e-3) / 1e9, "avg_us": b_ms * 1e3,
-                            "bytes_per_launch": B * BWD_BYTES},
-    }
-    for name, k in kernels.items():
-        k.update(peak=peak, unit="GB/s", frac=k["achieved"] / peak, traffic=ncu_traffic(name, B))
-    # the forward's second roofline: plain FP32 arithmetic.  Algorithmic work = 150 FP32 thread
-    # instructions per evaluation of T, g, Hessian and solve (eqs. (10)-(12)) x (mean updates + 1 final evaluation
-    # + 1 for the start-up steps); peak = 128 FP32 lanes per clock per SM at the maximum SM clock.
-    props = torch.cuda.get_device_properties(local)
-    sm_mhz = clocks.max_mhz or 1965
-    alu_peak = 128.0 * props.multi_processor_count * sm_mhz * 1e6 / 1e12
-    alu_work = 150.0 * (mean_updates + 2.0)
-    alu_ach = B * alu_work / (f_ms * 1e-3) / 1e12
-    kernels["forward_lean_kernel"]["alu"] = {
-        "bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T FP32 instr/s", "frac": alu_ach / alu_peak,
-        "fp32_instr_per_matrix": alu_work}
-    dom = "forward_lean_kernel" if f_ms >= b_ms else "backward_kernel"
-    roofline = dict(kernels[dom], kernel=dom, peak_source=peak_src)
+    fk = head["roofline_kernels"]["forward_kernel"]
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "desc": wl["desc"], "B_per_gpu": B, "tol": TOL, "max_iter": max_iter,
-                   "variant": args.variant,
                    "parallelism": "batch shards, no collective" if world > 1 else "single GPU",
-                   "l2": "rotation over %d buffer sets (%.2f GiB); backward reads the P written %d steps earlier"
-                         % (nsets, nsets * set_bytes / 2 ** 30, nsets - 1)},
-        "fwd": {"value": world * B / (f_ms * 1e-3), "unit": UNIT, "mean_newton_updates": mean_updates,
-                "update_histogram": update_hist,
-                "unconverged": int(unc.item())},
-        "max_marginal_err": max_err, "mean_marginal_err": mean_err,
-        "roofline": roofline, "roofline_kernels": kernels, "sinkhorn20_gpu": sink,
-        "e2e": e2e, "gpu_launches": 2 * K, "gpu_launches_per_kernel_timing": 2 * K, "clocks": clocks.summary(),
+                   "l2": "rotation over %d buffer sets (>= 1 GiB); backward reads the P written %d steps earlier"
+                         % (head["buffer_sets"], head["buffer_sets"] - 1),
+                   "repeats": "every per-kernel and per-step time is the median (and min) of %d regions of %d calls" % (R, K)},
+        # the dominant kernel is the forward (the Newton solver: the backward is a pure stream); its HBM roofline
+        "roofline": dict(fk, kernel="forward_kernel", peak_source=peak_src),
+        "roofline_step": head["roofline_step"], "roofline_kernels": head["roofline_kernels"],
+        "fwd": {"value": world * head["fwd_matrices_per_s"], "unit": UNIT, "us": head["forward_us"],
+                "mean_newton_updates": head["mean_newton_updates"], "update_histogram": head["update_histogram"],
+                "unconverged": head["unconverged"]},
+        "bwd": {"us": head["backward_us"]}, "step_us": head["step_us"],
+        "max_marginal_err": head["max_marginal_err"], "mean_marginal_err": head["mean_marginal_err"],
+        "max_err_inf": head["max_err_inf"], "sinkhorn20_gpu": sink, "e2e": e2e,
     }
+    if world == 1 and args.workload == "config2" and not args.no_extra:
+        clocks.region(True)
+        extra = {}
+        Kx, Rx = min(K, 20), min(R, 10)
+        for name, kw in (("config3_s10", {}), ("config3_s10@max_iter20", {"max_iter": 20}), ("config3_s30", {}),
+                         ("config3_s30@max_iter20", {"max_iter": 20}), ("config3_s100", {}),
+                         ("config3_s100@max_iter20", {"max_iter": 20}), ("config4", {}), ("config5", {}),
+                         ("config5@sorted_by_class", {"sort_by_class": True})):
+            base = name.split("@")[0]
+            res, s_, _ = measure_workload(torch, bk, inputs, base, WORKLOADS[base], 0, Kx, Rx, peak, peak_src, sm_mhz,
+                                          props.multi_processor_count, **kw)
+            launches += 3 * Kx * Rx
+            extra[name] = res
+            del s_
+            torch.cuda.empty_cache()
+        out["workloads"] = extra
+        out["widenings"] = measure_widenings(torch, bk, inputs, Kx, min(Rx, 5), peak)
+        clocks.region(False)
+    clocks.stop()
+    out["gpu_launches"] = launches
+    out["gpu_launches_timed_region"] = 2 * K
+    out["clocks"] = clocks.summary()
     if world == 1 and not args.no_cpu_baseline:
         import oracle
         n = min(B, 1 << 20 if wl["config"] in (2, 4) else 1 << 14)                # about 10 s of host work
@@ -380,8 +523,14 @@ def run_ours(args, wl):
         t0 = time.perf_counter()
         oracle_step(oracle, Hs, G0[:n])
         dt = time.perf_counter() - t0
+        n1 = max(1024, n // 16)
+        t0 = time.perf_counter()
+        oracle_step(oracle, Hs[:n1], G0[:n1], nthreads=1)
+        dt1 = time.perf_counter() - t0
         out["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                               "sample": "first %d matrices of buffer set 0, forward+backward, fp64, %.1f s" % (n, dt)}
+                               "sample": "first %d matrices of buffer set 0, forward+backward, fp64, %.1f s" % (n, dt),
+                               "one_thread": {"value": n1 / dt1, "unit": UNIT, "cores": 1,
+                                              "sample": "first %d matrices, %.1f s" % (n1, dt1)}}
     print(json.dumps(_finite(out)))
     if world > 1:
         dist.destroy_process_group()
@@ -390,12 +539,13 @@ def run_ours(args, wl):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1000)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--regions", type=int, default=10, help="timed regions of --steps calls per kernel (median and min reported)")
+    ap.add_argument("--no-extra", action="store_true", help="config2 only: skip the workloads / widenings blocks")
     ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--variant", type=int, default=0, help="forward kernel variant (0 = library default)")
     args = ap.parse_args()
     wl = WORKLOADS[args.workload]
     if args.impl == "reference":
