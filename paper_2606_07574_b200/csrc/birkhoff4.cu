@@ -165,7 +165,7 @@ static inline unsigned grid_for(int64_t B, int threads) { return (unsigned)((B +
 // The kernels test the column residual err = sum_m |g_m| computed in fp32 (rows sum to 1 by construction).  Err of
 // PAPER.md:323, evaluated exactly on the stored fp32 P, adds to it the rounding of the stored entries (up to half an
 // ulp of 1 in each of the 4 + 4 sums when P is close to a permutation) and the rounding of g itself: DESIGN.md S3/S9
-// budgets these at 0.5 tol for tol = 1e-6, so the tested threshold is 0.5 tol, and never more than tol - 5e-7.
+// budgets these at 0.5 tol for tol = 1e-6, so the tested threshold is 0.5 tol, or tol - 7e-7 if that is larger.
 static inline float internal_tol(float tol) {
     float f = 0.5f;
 #ifdef BK4_EXPERIMENTS

@@ -28,6 +28,7 @@ constexpr int kSmStride = BK4_THREADS;   // floats between consecutive entries o
 constexpr float kLeanFloor = 1e-5f;     // a residual that stalls below this is the fp32 floor, not a failure
 constexpr int kLeanSweeps = 3;          // start-up Sinkhorn sweeps of the narrow start
 constexpr int kLeanFree = 2;            // Newton updates taken before the first residual test
+constexpr int kLeanFreeWide = 3;        // the same when every matrix of the warp took the wide start
 static_assert(kLeanFree == 2, "lean_iterate spells the free updates out");
 constexpr float kPeakedSum = 1.05f;     // every row sum of exp(H - rowmax) below this: wide start (see narrow_exponentials)
 constexpr int kLeanNoisy = 4;            // tested updates during which a residual within 4 tol_i may rise
@@ -235,11 +236,20 @@ struct LeanResult {
 //     result and T is handed back once.
 // A lane that is not `active` only follows the warp.  `stored` is false for a matrix whose residual stopped falling
 // above the fp32 floor (and for NaN): the guarded solver takes it.
-BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, float tol_i, int max_iter,
-                                float (&T)[16]) {
+// all_wide (the same for every lane of the warp): no lane took the narrow start.  After the wide start half of the
+// matrices need a third update and a quarter a fourth, so the warp takes kLeanFreeWide plain updates before the first
+// test instead of kLeanFree with the last one refined.
+BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, bool all_wide, float tol_i,
+                                int max_iter, float (&T)[16]) {
     float g[4];
     int it = 0;
-    if (max_iter >= kLeanFree) {
+    if (all_wide && max_iter >= kLeanFreeWide) {
+#pragma unroll 1
+        for (; it < kLeanFreeWide; ++it) {
+            eval_T<false>(E, v0, v1, v2, T, g);
+            lean_update<false>(T, g, true, v0, v1, v2);
+        }
+    } else if (max_iter >= kLeanFree) {
         // (the last free update is the last update of nearly every well-scaled matrix: refined reciprocal and
         // accurate exponential, or the 2^-23 of the SFU reciprocal is left in the residual for the test to find)
         eval_T<false>(E, v0, v1, v2, T, g);

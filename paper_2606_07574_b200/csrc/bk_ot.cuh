@@ -55,6 +55,19 @@ BK4_DEV void store_row(float* p, const float (&r)[K]) {
     }
 }
 
+// all N rows of one problem: the loads are issued back to back (a load followed by arithmetic on it, row after row,
+// would leave one row in flight per thread and bind the kernel by latency)
+template <int N, int M>
+BK4_DEV void load_all(const float* p, float (&X)[N * M]) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float r[M];
+        load_row<M>(p + i * M, r);
+#pragma unroll
+        for (int j = 0; j < M; ++j) X[i * M + j] = r[j];
+    }
+}
+
 // index of the edge weight W_jk, j < k < M, in the packed upper triangle
 template <int M>
 BK4_DEV constexpr int tri(int j, int k) {
@@ -153,21 +166,21 @@ BK4_DEV void ot_eval(const float (&E)[N * M], const float (&v)[M - 1], const flo
     }
 }
 
-// E_ij = exp((beta_j - C_ij) / eta - mu_i) for the base potentials beta (beta_{M-1} = 0), mu_i the row maximum.
-// sign = -1 for costs C (entropic OT), +1 for logits H = -C (Birkhoff projection).  Returns false if a NaN/Inf
-// was met.
+// E_ij = exp((beta_j - C_ij) / eta - mu_i) for the base potentials beta (beta_{M-1} = 0), mu_i the row maximum; E holds
+// the raw costs (or logits) on entry.  sign = -1 for costs C (entropic OT), +1 for logits H = -C (Birkhoff
+// projection).  Returns false if a NaN/Inf was met.
 template <int N, int M>
-BK4_DEV bool ot_exponentials(const float* Cg, float sign_over_eta, const float (&beta_over_eta)[M - 1], float (&E)[N * M]) {
+BK4_DEV bool ot_exponentials(float sign_over_eta, const float (&beta_over_eta)[M - 1], float (&E)[N * M]) {
     float poison = 0.0f;
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        float row[M], u[M];
-        load_row<M>(Cg + i * M, row);
+        float u[M];
         float mx = -kInf;
 #pragma unroll
         for (int j = 0; j < M; ++j) {
-            poison = __fmaf_rn(row[j], 0.0f, poison);
-            u[j] = j < M - 1 ? fmaf(row[j], sign_over_eta * kLog2e, beta_over_eta[j]) : row[j] * (sign_over_eta * kLog2e);
+            const float c = E[i * M + j];
+            poison = __fmaf_rn(c, 0.0f, poison);
+            u[j] = j < M - 1 ? fmaf(c, sign_over_eta * kLog2e, beta_over_eta[j]) : c * (sign_over_eta * kLog2e);
             mx = fmaxf(mx, u[j]);
         }
 #pragma unroll
@@ -190,14 +203,13 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
     float E[N * M], v[M - 1], vprev[M - 1], bl[M - 1], c[M], W[M * (M - 1) / 2];
     // range of the costs decides the continuation schedule
     float lo = kInf, hi = -kInf, suma = 0.0f;
+    load_all<N, M>(Cg, E);
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        float row[M];
-        load_row<M>(Cg + i * M, row);
 #pragma unroll
         for (int j = 0; j < M; ++j) {
-            lo = fminf(lo, row[j]);
-            hi = fmaxf(hi, row[j]);
+            lo = fminf(lo, E[i * M + j]);
+            hi = fmaxf(hi, E[i * M + j]);
         }
         suma += UNIT ? 1.0f : a[i];
     }
@@ -212,8 +224,9 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
     for (int j = 0; j < M - 1; ++j) bl[j] = 0.0f;  // base potentials / eta_s in log2 units
     OtStats st = {0, false};
     bool finite = true;
-    for (;; eta_s *= 0.5f, --stages) {
-        finite = ot_exponentials<N, M>(Cg, sign / eta_s, bl, E) && finite;
+    for (bool first = true;; eta_s *= 0.5f, --stages, first = false) {
+        if (!first) load_all<N, M>(Cg, E);  // a later stage: the costs again (through L2)
+        finite = ot_exponentials<N, M>(sign / eta_s, bl, E) && finite;
 #pragma unroll
         for (int j = 0; j < M - 1; ++j) v[j] = 1.0f;
         // Sinkhorn sweeps in the scaling form of eq. (2) PAPER.md:76 with marginals: u = a / (E v), v = b / (E^T u)
@@ -315,6 +328,8 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
 template <int N, int M>
 BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, float* Dg) {
     float T[N * M], G[N * M], W[M * (M - 1) / 2], mur[N], ia[N], rhs[M], w[M - 1];
+    load_all<N, M>(Tg, T);
+    load_all<N, M>(Gg, G);  // D may alias G: all of G is in registers before anything is written
 #pragma unroll
     for (int q = 0; q < M * (M - 1) / 2; ++q) W[q] = 0.0f;
 #pragma unroll
@@ -322,16 +337,11 @@ BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, 
     float suma = 0.0f;
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        float t[M], g[M];
-        load_row<M>(Tg + i * M, t);
-        load_row<M>(Gg + i * M, g);
         float ai = 0.0f, mr = 0.0f;
 #pragma unroll
         for (int j = 0; j < M; ++j) {
-            T[i * M + j] = t[j];
-            G[i * M + j] = g[j];
-            ai += t[j];
-            mr = fmaf(g[j], t[j], mr);
+            ai += T[i * M + j];
+            mr = fmaf(G[i * M + j], T[i * M + j], mr);
         }
         suma += ai;
         ia[i] = rcp_approx(ai);
@@ -339,12 +349,12 @@ BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, 
         mur[i] = mr;
         const float mra = mr * ia[i];
 #pragma unroll
-        for (int j = 0; j < M; ++j) rhs[j] += fmaf(g[j], t[j], -t[j] * mra);  // mu_c_j - sum_i T_ij mu_r_i / a_i
+        for (int j = 0; j < M; ++j) rhs[j] += fmaf(G[i * M + j], T[i * M + j], -T[i * M + j] * mra);  // mu_c_j - sum_i T_ij mu_r_i / a_i
 #pragma unroll
         for (int j = 0; j < M - 1; ++j) {
-            const float tj = t[j] * ia[i];
+            const float tj = T[i * M + j] * ia[i];
 #pragma unroll
-            for (int k = j + 1; k < M; ++k) W[tri<M>(j, k)] = fmaf(tj, t[k], W[tri<M>(j, k)]);
+            for (int k = j + 1; k < M; ++k) W[tri<M>(j, k)] = fmaf(tj, T[i * M + k], W[tri<M>(j, k)]);
         }
     }
     float gneg[M];
@@ -353,11 +363,10 @@ BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, 
     solve_laplacian<M>(W, gneg, kOtLam * suma * (1.0f / N), w);
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        float tw = 0.0f;
+        float tw = 0.0f, d[M];
 #pragma unroll
         for (int j = 0; j < M - 1; ++j) tw = fmaf(T[i * M + j], w[j], tw);
         const float vi = (mur[i] - tw) * ia[i];
-        float d[M];
 #pragma unroll
         for (int j = 0; j < M; ++j) d[j] = out_scale * T[i * M + j] * ((vi - G[i * M + j]) + (j < M - 1 ? w[j] : 0.0f));
         store_row<M>(Dg + i * M, d);
