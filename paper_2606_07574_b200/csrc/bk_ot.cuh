@@ -18,6 +18,8 @@
 // 24-permutation brute force): wide costs are reached by continuation in eta (eps-scaling): the problem is solved
 // at eta 2^K, ..., 2 eta, eta with 2^K eta ~ range / 8, each stage started from the potentials of the one before.
 #pragma once
+#include <type_traits>
+
 #include "bk4_math.cuh"
 
 namespace bkot {
@@ -74,56 +76,70 @@ BK4_DEV constexpr int tri(int j, int k) {
     return j * M - j * (j + 1) / 2 + (k - j - 1);
 }
 
+// compile-time loop: f(integral_constant<int, I>) for I = Begin .. End-1.  (With a plain `#pragma unroll` nest nvcc 12.9
+// gives up on the elimination below for M = 8 and indexes W in local memory.)
+template <int I, int End, class F>
+BK4_DEV void static_for(F&& f) {
+    if constexpr (I < End) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, End>(f);
+    }
+}
+
 // Solve the grounded Laplacian system L d = -g, L_jk = -W_jk (j != k), L_jj = sum_{k != j} W_jk, unknowns j < M-1,
 // ground = column M-1 (its links get `lam`), by node elimination in the order 0, 1, ...  W (packed) is destroyed.
+// Eliminating node p gives its neighbours j, k > p the weight W_jk += W_pj W_pk / deg_p; the new degree of j is
+// recomputed as the sum of its remaining weights, all non-negative: no subtraction anywhere (S7).
 template <int M>
 BK4_DEV void solve_laplacian(float (&W)[M * (M - 1) / 2], const float (&g)[M], float lam, float (&d)[M - 1]) {
     constexpr int K = M - 1;
     float deg[K], rhs[K], inv[K];
-#pragma unroll
-    for (int j = 0; j < K; ++j) {
+    static_for<0, K>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
         W[tri<M>(j, K)] += lam;
+    });
+    static_for<0, K>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
         float s = 0.0f;
-#pragma unroll
-        for (int k = 0; k < M; ++k)
-            if (k != j) s += W[k > j ? tri<M>(j, k) : tri<M>(k, j)];
+        static_for<0, M>([&](auto kc) {
+            constexpr int k = decltype(kc)::value;
+            if constexpr (k != j) s += W[k > j ? tri<M>(j, k) : tri<M>(k, j)];
+        });
         deg[j] = s;
         rhs[j] = -g[j];
-    }
-    // eliminate node p: for its neighbours j, k > p:  W_jk += W_pj W_pk / deg_p,  deg_j -= W_pj - (W_pj / deg_p)(deg_p - W_pj) ...
-    // written through the degrees: deg_j' = sum of the new weights of j, which is deg_j - W_pj^2 / deg_p  (the link
-    // to p goes, the links it gains sum to W_pj (deg_p - W_pj) / deg_p)
-#pragma unroll
-    for (int p = 0; p < K; ++p) {
+    });
+    static_for<0, K>([&](auto pc) {
+        constexpr int p = decltype(pc)::value;
         inv[p] = rcp_approx(deg[p]);
-#pragma unroll
-        for (int j = p + 1; j < K; ++j) {
+        static_for<p + 1, K>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
             const float f = W[tri<M>(p, j)] * inv[p];
-#pragma unroll
-            for (int k = j + 1; k < M; ++k) W[tri<M>(j, k)] = fmaf(f, W[tri<M>(p, k)], W[tri<M>(j, k)]);
-            // new degree of j: recomputed from non-negative terms below (no subtraction)
+            static_for<j + 1, M>([&](auto kc) {
+                constexpr int k = decltype(kc)::value;
+                W[tri<M>(j, k)] = fmaf(f, W[tri<M>(p, k)], W[tri<M>(j, k)]);
+            });
             rhs[j] = fmaf(f, rhs[p], rhs[j]);
-        }
-#pragma unroll
-        for (int j = p + 1; j < K; ++j) {
-            // links of j to the nodes before it are gone; its degree is the sum over what is left plus what it gained
-            // through p: sum_{k > p, k != j} W'_jk.  The weights W'_jk for k < j were updated symmetrically above
-            // (stored at tri(k, j)), so the sum runs over the packed triangle.
+        });
+        static_for<p + 1, K>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
             float s = 0.0f;
-#pragma unroll
-            for (int k = p + 1; k < M; ++k)
-                if (k != j) s += W[k > j ? tri<M>(j, k) : tri<M>(k, j)];
+            static_for<p + 1, M>([&](auto kc) {
+                constexpr int k = decltype(kc)::value;
+                if constexpr (k != j) s += W[k > j ? tri<M>(j, k) : tri<M>(k, j)];
+            });
             deg[j] = s;
-        }
-    }
+        });
+    });
     // back substitution: d_p = (rhs_p + sum_{k > p, k < K} W_pk d_k) / deg_p
-#pragma unroll
-    for (int p = K - 1; p >= 0; --p) {
+    static_for<0, K>([&](auto qc) {
+        constexpr int p = K - 1 - decltype(qc)::value;
         float s = rhs[p];
-#pragma unroll
-        for (int k = p + 1; k < K; ++k) s = fmaf(W[tri<M>(p, k)], d[k], s);
+        static_for<p + 1, K>([&](auto kc) {
+            constexpr int k = decltype(kc)::value;
+            s = fmaf(W[tri<M>(p, k)], d[k], s);
+        });
         d[p] = s * inv[p];
-    }
+    });
 }
 
 // One streamed evaluation at v: column sums c_j = sum_i T_ij, and (HESS) the packed edge weights
