@@ -124,12 +124,8 @@ __global__ void __launch_bounds__(kThreads, 512 / kThreads) forward_mix_kernel(
     __syncthreads();
     // phase 2: the block streams its tokens' 4 x C activations
     const int ntok = (int)((B - tok0 < kMixTokens) ? B - tok0 : kMixTokens);
-    for (int t = 0; t < ntok; ++t) {
-        float p[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) p[q] = s_col[q * kSmStride + t];  // the same address for every thread: a broadcast
-        mix_token<XBF16>(p, X + (size_t)(tok0 + t) * 4 * C, Y + (size_t)(tok0 + t) * 4 * C, C);
-    }
+    for (int t = 0; t < ntok; t += kMixGroup)
+        mix_tokens<XBF16>(s_col, t, ntok - t, X + (size_t)(tok0 + t) * 4 * C, Y + (size_t)(tok0 + t) * 4 * C, C);
 }
 
 // ---------------------------------------------------------------- backward kernel (HBM-bound: 192 B per matrix)

@@ -5,7 +5,8 @@
 //
 // One block = kMixTokens tokens.  Phase 1: thread t projects token t's matrix (project_one: the same code as
 // birkhoff4_forward) and leaves P_t in its shared-memory column.  Phase 2: the block streams the tokens' 4 x C
-// activations: every thread reads P_t (a broadcast) and mixes a 16-byte slice of each of the four streams.
+// activations, kMixGroup tokens at a time: every thread reads P_t (a broadcast) and mixes a 16-byte slice of each of the
+// four streams, with the loads of the whole group in flight together.
 #pragma once
 #include <cuda_bf16.h>
 
@@ -21,6 +22,9 @@ template <>
 struct MixVec<false> {  // fp32 activations: 4 elements per 16-byte access
     static constexpr int kElems = 4;
     using elem = float;
+    using raw = float4;
+    BK4_DEV static raw load_raw(const float* p) { return __ldcs(reinterpret_cast<const float4*>(p)); }
+    BK4_DEV static void widen(const raw& t, float (&x)[4]) { x[0] = t.x, x[1] = t.y, x[2] = t.z, x[3] = t.w; }
     BK4_DEV static void load(const float* p, float (&x)[4]) {
         const float4 t = __ldcs(reinterpret_cast<const float4*>(p));
         x[0] = t.x, x[1] = t.y, x[2] = t.z, x[3] = t.w;
@@ -33,6 +37,16 @@ template <>
 struct MixVec<true> {  // bf16 activations (bit patterns): 8 elements per 16-byte access, fp32 accumulation
     static constexpr int kElems = 8;
     using elem = uint16_t;
+    using raw = uint4;
+    BK4_DEV static raw load_raw(const uint16_t* p) { return __ldcs(reinterpret_cast<const uint4*>(p)); }
+    BK4_DEV static void widen(const raw& t, float (&x)[8]) {
+        const uint32_t w[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            x[2 * k] = __uint_as_float(w[k] << 16);
+            x[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+        }
+    }
     BK4_DEV static void load(const uint16_t* p, float (&x)[8]) {
         const uint4 t = __ldcs(reinterpret_cast<const uint4*>(p));
         const uint32_t w[4] = {t.x, t.y, t.z, t.w};
@@ -53,22 +67,41 @@ struct MixVec<true> {  // bf16 activations (bit patterns): 8 elements per 16-byt
     }
 };
 
-// phase 2 for one token: y_i = sum_j P_ij x_j over this thread's slices of the C columns
+// phase 2 for kMixGroup consecutive tokens (`n` of them exist): y_i = sum_j P_ij x_j over this thread's slices of the C
+// columns.  All the group's loads (kMixGroup x 4 streams x 16 bytes per thread) are issued before the first is used:
+// with four blocks of 128 threads per SM that is what keeps enough bytes in flight to fill HBM (one token at a time
+// left 64 bytes per thread in flight and the kernel at 0.77 of the copy bandwidth; two: 0.92).  sP: the block's results, entry q
+// of token t at [q * kSmStride + t] (read as a broadcast).
+constexpr int kMixGroup = 2;  // measured: 1 / 2 / 3 / 4 tokens per group: 214 / 179 / 191 / 192 us (B = 2^16, C = 1024 bf16)
 template <bool XBF16>
-BK4_DEV void mix_token(const float (&p)[16], const typename MixVec<XBF16>::elem* x, typename MixVec<XBF16>::elem* y, int C) {
-    constexpr int V = MixVec<XBF16>::kElems;
+BK4_DEV void mix_tokens(const float* sP, int t0, int n, const typename MixVec<XBF16>::elem* x, typename MixVec<XBF16>::elem* y, int C) {
+    using MV = MixVec<XBF16>;
+    constexpr int V = MV::kElems;
     for (int c = threadIdx.x * V; c < C; c += kMixTokens * V) {
-        float xin[4][V], yout[V];
+        typename MV::raw in[kMixGroup][4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) MixVec<XBF16>::load(x + (size_t)j * C + c, xin[j]);
+        for (int g = 0; g < kMixGroup; ++g)
+            if (g < n) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+                for (int j = 0; j < 4; ++j) in[g][j] = MV::load_raw(x + ((size_t)g * 4 + j) * C + c);
+            }
 #pragma unroll
-            for (int e = 0; e < V; ++e)
-                yout[e] = fmaf(p[4 * i + 3], xin[3][e],
-                               fmaf(p[4 * i + 2], xin[2][e], fmaf(p[4 * i + 1], xin[1][e], p[4 * i] * xin[0][e])));
-            MixVec<XBF16>::store(y + (size_t)i * C + c, yout);
-        }
+        for (int g = 0; g < kMixGroup; ++g)
+            if (g < n) {
+                float p[16], xin[4][V], yout[V];
+#pragma unroll
+                for (int q = 0; q < 16; ++q) p[q] = sP[q * kSmStride + t0 + g];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) MV::widen(in[g][j], xin[j]);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e)
+                        yout[e] = fmaf(p[4 * i + 3], xin[3][e],
+                                       fmaf(p[4 * i + 2], xin[2][e], fmaf(p[4 * i + 1], xin[1][e], p[4 * i] * xin[0][e])));
+                    MV::store(y + ((size_t)g * 4 + i) * C + c, yout);
+                }
+            }
     }
 }
 
