@@ -229,34 +229,52 @@ struct LeanResult {
 
 // Free updates and tested iterations in warp lockstep (PAPER.md:164-168 with the guard of DESIGN.md S2 reduced to its
 // test: an update after which the column residual did not fall ends the lean iteration for that matrix).
-//   - the first min(kLeanFree, max_iter) updates are taken without looking at the residual: on well-scaled inputs
-//     no matrix is done before them, and whatever they produce is judged by the tested iterations;
-//   - then: evaluate, stop test, Newton update, until no lane is running.  The update count `it` is the same for
-//     every running lane.  A lane whose matrix is finished keeps its v, so the last evaluation is every lane's
-//     result and T is handed back once.
+//   - free updates, taken without looking at the residual (on well-scaled inputs no matrix is done before them, and
+//     whatever they produce is judged by the tested iterations).  How many is a property of the MATRIX:
+//       plain3 (wide start and max_iter >= kLeanFreeWide): kLeanFreeWide plain updates: after the wide start half of
+//         the matrices need a third update and a quarter a fourth;
+//       otherwise: min(kLeanFree, max_iter) updates, the last one refined (it is the last update of nearly every
+//         well-scaled matrix: refined reciprocal and accurate exponential, or the 2^-23 of the SFU reciprocal is left
+//         in the residual for the test to find).
+//     A warp whose matrices all agree runs that schedule; a warp that holds both kinds runs the merged one, in which
+//     every lane gets exactly the arithmetic of its own schedule (eval_T_sel, exp_step_sel), so a matrix's result does
+//     not depend on its warp neighbours.
+//   - then: evaluate, stop test, Newton update, until no lane is running.  A lane whose matrix is finished keeps its
+//     v, so the last evaluation is every lane's result and T is handed back once.
 // A lane that is not `active` only follows the warp.  `stored` is false for a matrix whose residual stopped falling
 // above the fp32 floor (and for NaN): the guarded solver takes it.
-// all_wide (the same for every lane of the warp): no lane took the narrow start.  After the wide start half of the
-// matrices need a third update and a quarter a fourth, so the warp takes kLeanFreeWide plain updates before the first
-// test instead of kLeanFree with the last one refined.
-BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, bool all_wide, float tol_i,
+BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, bool plain3, float tol_i,
                                 int max_iter, float (&T)[16]) {
     float g[4];
-    int it = 0;
-    if (all_wide && max_iter >= kLeanFreeWide) {
+    int it = 0;  // this lane's update count
+    const bool any3 = __any_sync(0xffffffffu, plain3), all3 = __all_sync(0xffffffffu, plain3 || !active);
+    if (any3 && all3) {
 #pragma unroll 1
         for (; it < kLeanFreeWide; ++it) {
             eval_T<false>(E, v0, v1, v2, T, g);
             lean_update<false>(T, g, true, v0, v1, v2);
         }
-    } else if (max_iter >= kLeanFree) {
-        // (the last free update is the last update of nearly every well-scaled matrix: refined reciprocal and
-        // accurate exponential, or the 2^-23 of the SFU reciprocal is left in the residual for the test to find)
+    } else if (!any3 && max_iter >= kLeanFree) {
         eval_T<false>(E, v0, v1, v2, T, g);
         lean_update<false>(T, g, true, v0, v1, v2);
         eval_T<true, false>(E, v0, v1, v2, T, g);
         lean_update<true>(T, g, true, v0, v1, v2);
         it = kLeanFree;
+    } else if (any3) {
+        // merged schedule (max_iter >= kLeanFreeWide here): update 1 plain for everyone; update 2 plain for plain3 lanes,
+        // refined for the others; update 3 for plain3 lanes only
+        static_assert(kLeanFreeWide == kLeanFree + 1, "the merged schedule spells the updates out");
+        eval_T<false>(E, v0, v1, v2, T, g);
+        lean_update<false>(T, g, true, v0, v1, v2);
+        eval_T_sel(E, v0, v1, v2, !plain3, T, g);
+        {
+            float d1, d2, d3;
+            newton_direction<true>(T, g[0], g[1], g[2], d1, d2, d3);
+            v0 *= exp_step_sel(d1, !plain3), v1 *= exp_step_sel(d2, !plain3), v2 *= exp_step_sel(d3, !plain3);
+        }
+        eval_T<false>(E, v0, v1, v2, T, g);
+        lean_update<false>(T, g, plain3, v0, v1, v2);
+        it = plain3 ? kLeanFreeWide : kLeanFree;
     } else {
         for (; it < max_iter; ++it) {
             eval_T<false>(E, v0, v1, v2, T, g);

@@ -61,7 +61,7 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
                 } else {
                     code = kIdentityCode;
                 }
-                res = lean_iterate(E, v0, v1, v2, active, !any_narrow, tol_i, max_iter, T);
+                res = lean_iterate(E, v0, v1, v2, active, wide && max_iter >= kLeanFreeWide, tol_i, max_iter, T);
                 if (active && res.stored) {
                     float out[16];
                     unpermute_columns(T, code, sm, out);

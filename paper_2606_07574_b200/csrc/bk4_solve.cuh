@@ -97,6 +97,34 @@ BK4_DEV void eval_T(const float (&E)[16], float v0, float v1, float v2, float (&
     if constexpr (!ALL4) g[3] = 0.0f;
 }
 
+// eval_T<true, false> for the lanes with `refine`, eval_T<false> for the others, bit for bit, in one instruction stream
+// (a warp that holds both kinds of matrices: DESIGN.md S1): the refinement r += r (1 - sum r) is multiplied by 0 or 1.
+BK4_DEV void eval_T_sel(const float (&E)[16], float v0, float v1, float v2, bool refine, float (&T)[16], float (&g)[4]) {
+    const float m = refine ? 1.0f : 0.0f;
+    float out[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float x[4] = {E[4 * i] * v0, E[4 * i + 1] * v1, E[4 * i + 2] * v2, E[4 * i + 3]};
+        const int a = (i + 1) & 3, b = (i + 2) & 3, c = (i + 3) & 3;
+        const float off = (x[a] + x[b]) + x[c];
+        const float sum = x[i] + off;
+        float r = rcp_approx(sum);
+        r = fmaf(r * m, fmaf(-sum, r, 1.0f), r);  // refine: fmaf(r, e, r); else: fmaf(0, e, r) = r
+        T[4 * i + a] = x[a] * r;
+        T[4 * i + b] = x[b] * r;
+        T[4 * i + c] = x[c] * r;
+        out[i] = off * r;
+        const float diag = 1.0f - out[i];
+        T[5 * i] = refine ? fmaxf(diag, 0.0f) : diag;
+    }
+#pragma unroll
+    for (int mcol = 0; mcol < 3; ++mcol) {
+        const int a = (mcol + 1) & 3, b = (mcol + 2) & 3, c = (mcol + 3) & 3;
+        g[mcol] = ((T[4 * a + mcol] + T[4 * b + mcol]) + T[4 * c + mcol]) - out[mcol];
+    }
+    g[3] = 0.0f;
+}
+
 // beta += d  <=>  v *= exp(d).  ACCURATE (updates that may be the last): for |d| < 2^-8 the factor is
 // 1 + d + d^2/2 (error below 2^-26) instead of the SFU's exp (relative error 2^-22, which at the end of the
 // iteration is the largest error in v).
@@ -106,6 +134,12 @@ BK4_DEV float exp_step(float d) {
     if constexpr (!ACCURATE) return e;
     const float p = fmaf(d, fmaf(d, 0.5f, 1.0f), 1.0f);
     return fabsf(d) < 0.00390625f ? p : e;
+}
+// exp_step<true> for the lanes with `accurate`, exp_step<false> for the others
+BK4_DEV float exp_step_sel(float d, bool accurate) {
+    const float e = ex2_approx(d * kLog2e);
+    const float p = fmaf(d, fmaf(d, 0.5f, 1.0f), 1.0f);
+    return (accurate && fabsf(d) < 0.00390625f) ? p : e;
 }
 
 // -------------------------------------------------------------------------------------------------

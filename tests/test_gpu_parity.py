@@ -314,6 +314,24 @@ def test_result_depends_on_the_matrix_alone():
     assert np.array_equal(gpu_forward(H, max_iter=32), P)                        # deterministic
 
 
+@pytest.mark.parametrize("max_iter", [32, 3, 2])
+def test_schedule_of_free_updates_is_per_matrix(max_iter):
+    """a wide matrix takes three plain untested updates and a narrow one two (S1/S2) whatever shares its warp:
+    warps of wide matrices only, of narrow ones only, alternating ones, and one stranger per warp give the same bits"""
+    n = 1 << 13
+    W = inputs.normal(n, 30.0, config=3, sub=5)[0]
+    N = inputs.normal(n, 1.0, config=2, sub=5)[0]
+    PW, PN = gpu_forward(W, max_iter=max_iter), gpu_forward(N, max_iter=max_iter)
+    mix = np.empty((2 * n, 4, 4), np.float32)
+    mix[0::2], mix[1::2] = W, N
+    PM = gpu_forward(mix, max_iter=max_iter)
+    assert np.array_equal(PM[0::2], PW) and np.array_equal(PM[1::2], PN)
+    for host, guest, Ph, Pg in ((W, N, PW, PN), (N, W, PN, PW)):
+        sp, exp = host.copy(), Ph.copy()
+        sp[5::32], exp[5::32] = guest[5::32], Pg[5::32]
+        assert np.array_equal(gpu_forward(sp, max_iter=max_iter), exp)
+
+
 def test_guarded_solver_agrees_on_mixed_batch():
     H = dev(_mixed_batch(1 << 15, seed=75))
     a = bk.birkhoff4_forward(H, max_iter=32)
