@@ -16,7 +16,7 @@
 // What is different: rows are streamed (T is never held whole: with N M = 64 entries the registers hold E, the
 // column sums and the M(M-1)/2 edge weights); there is no LP start (an assignment problem for N = M = 8 has no
 // 24-permutation brute force): wide costs are reached by continuation in eta (eps-scaling): the problem is solved
-// at eta 2^K, ..., 2 eta, eta with 2^K eta ~ range / 8, each stage started from the potentials of the one before.
+// at eta 2^K, ..., 2 eta, eta with 2^K eta ~ range / 16, each stage started from the potentials of the one before.
 #pragma once
 #include <type_traits>
 
@@ -28,7 +28,7 @@ using namespace bk4;
 
 constexpr float kOtLam = 2.384185791015625e-07f;  // ground regularisation, relative to the mean row marginal
 constexpr int kOtSweeps = 3;                     // Sinkhorn sweeps at the start of every continuation stage
-constexpr float kOtStageRange = 8.0f;            // a stage's scaled costs span at most this
+constexpr float kOtStageRange = 16.0f;           // a stage's scaled costs span at most this (8 / 12 / 16 / 20 / 24 measured: DESIGN.md)
 constexpr int kOtHalvings = 4;                   // step halvings before the Sinkhorn fallback
 constexpr float kOtStageTol = 1e-2f;             // relative marginal error at which an intermediate stage is left
 
