@@ -205,6 +205,26 @@ BK4_DEV bool ot_exponentials(float sign_over_eta, const float (&beta_over_eta)[M
     return poison == 0.0f;
 }
 
+// One Sinkhorn sweep in scaling form: u_i = a_i / sum_j E_ij v_j, q_j = sum_i E_ij u_i, v_j = (b_j / q_j) / (b_M / q_M).
+template <int N, int M, bool UNIT>
+BK4_DEV void ot_sweep(const float (&E)[N * M], float (&v)[M - 1], const float (&a)[N], const float (&b)[M]) {
+    float q[M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) q[j] = 0.0f;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        float s = E[i * M + M - 1];
+#pragma unroll
+        for (int j = 0; j < M - 1; ++j) s = fmaf(E[i * M + j], v[j], s);
+        const float u = UNIT ? rcp_approx(s) : a[i] * rcp_approx(s);
+#pragma unroll
+        for (int j = 0; j < M; ++j) q[j] = fmaf(E[i * M + j], u, q[j]);
+    }
+    const float t = UNIT ? q[M - 1] : q[M - 1] * rcp_approx(b[M - 1]);  // 1 / v_M before the gauge
+#pragma unroll
+    for (int j = 0; j < M - 1; ++j) v[j] = (UNIT ? t : b[j] * t) * rcp_approx(q[j]);
+}
+
 struct OtStats {
     int iters;
     bool converged;
@@ -245,13 +265,9 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
         finite = ot_exponentials<N, M>(sign / eta_s, bl, E) && finite;
 #pragma unroll
         for (int j = 0; j < M - 1; ++j) v[j] = 1.0f;
-        // Sinkhorn sweeps in the scaling form of eq. (2) PAPER.md:76 with marginals: u = a / (E v), v = b / (E^T u)
-        for (int k = 0; k < kOtSweeps; ++k) {
-            ot_eval<N, M, UNIT, false>(E, v, a, c, W);
-            const float t = (UNIT ? 1.0f : b[M - 1]) * rcp_approx(c[M - 1]);
-#pragma unroll
-            for (int j = 0; j < M - 1; ++j) v[j] *= (UNIT ? 1.0f : b[j]) * rcp_approx(c[j] * t);
-        }
+        // Sinkhorn sweeps in the scaling form of eq. (2) PAPER.md:76 with marginals: u = a / (E v), v = b / (E^T u), gauge
+        // v_M = 1 (two fused multiply-adds per entry; T itself is not formed)
+        for (int k = 0; k < kOtSweeps; ++k) ot_sweep<N, M, UNIT>(E, v, a, b);
         const float tol_s = stages > 0 ? kOtStageTol * suma : tol_abs;
         float errprev = kInf, tstep = 1.0f, d[M - 1];
         unsigned newton_trial = 0u, sink_trial = 0u;
