@@ -197,7 +197,7 @@ static int launch_forward(const void* H, float* P, int64_t B, float tol, int max
 // ---- host-buffer path: a ring of device buffers and streams; chunked H2D -> kernels -> D2H
 struct HostRing {
     static constexpr int kSlots = 3;
-    static constexpr int64_t kChunk = 1 << 18;  // matrices per chunk (16 MiB per fp32 tensor)
+    static constexpr int64_t kChunk = 1 << 17;  // matrices per chunk (8 MiB per fp32 tensor; 2^16 / 2^17 / 2^18 measured: DESIGN.md)
     bool ready = false;
     int device = -1;
     cudaStream_t stream[kSlots] = {};
@@ -263,15 +263,24 @@ static int run_host(const float* H_host, const float* P_in_host, const float* dP
         cudaStream_t st = g_ring.stream[slot];
         float *dHm = g_ring.buf[slot][0], *dG = g_ring.buf[slot][1], *dPm = g_ring.buf[slot][2],
               *dD = g_ring.buf[slot][3];
+        if (mode == 3) {
+            // forward + backward: both inputs up, the fused kernel (P stays in registers between the two halves), both results down
+            rc = cuda_rc(cudaMemcpyAsync(dHm, H_host + 16 * off, bytes, cudaMemcpyHostToDevice, st));
+            if (!rc) rc = cuda_rc(cudaMemcpyAsync(dG, dP_host + 16 * off, bytes, cudaMemcpyHostToDevice, st));
+            if (!rc)
+                rc = launch_forward<false, false, true>(dHm, P_host ? dPm : nullptr, n, tol, max_iter, FwdDiag{nullptr, nullptr, nullptr}, st,
+                                                        FusedBwd{dG, dD});
+            if (!rc && P_host) rc = cuda_rc(cudaMemcpyAsync(P_host + 16 * off, dPm, bytes, cudaMemcpyDeviceToHost, st));
+            if (!rc) rc = cuda_rc(cudaMemcpyAsync(dH_host + 16 * off, dD, bytes, cudaMemcpyDeviceToHost, st));
+            continue;
+        }
         if (mode & 1) {
             rc = cuda_rc(cudaMemcpyAsync(dHm, H_host + 16 * off, bytes, cudaMemcpyHostToDevice, st));
             if (!rc) rc = launch_forward<false>(dHm, dPm, n, tol, max_iter, FwdDiag{nullptr, nullptr, nullptr}, st);
             if (!rc && P_host) rc = cuda_rc(cudaMemcpyAsync(P_host + 16 * off, dPm, bytes, cudaMemcpyDeviceToHost, st));
         } else {
             rc = cuda_rc(cudaMemcpyAsync(dPm, P_in_host + 16 * off, bytes, cudaMemcpyHostToDevice, st));
-        }
-        if (!rc && (mode & 2)) {
-            rc = cuda_rc(cudaMemcpyAsync(dG, dP_host + 16 * off, bytes, cudaMemcpyHostToDevice, st));
+            if (!rc) rc = cuda_rc(cudaMemcpyAsync(dG, dP_host + 16 * off, bytes, cudaMemcpyHostToDevice, st));
             if (!rc) rc = birkhoff4_backward(dPm, dG, dD, n, st);
             if (!rc) rc = cuda_rc(cudaMemcpyAsync(dH_host + 16 * off, dD, bytes, cudaMemcpyDeviceToHost, st));
         }
