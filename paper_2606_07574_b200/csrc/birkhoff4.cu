@@ -82,6 +82,13 @@ __global__ void __launch_bounds__(kThreads, 1024 / kThreads) forward_kernel(cons
     };
     // the result of this thread's matrix (original column order): store it and, when fused, differentiate it
     auto commit = [&](const float(&out)[16]) {
+        // (the matrix index is formed again from the special registers: kept from the top of the kernel it is the one
+        // value that does not fit 64 registers, and its spill costs every thread 8 bytes of L2 write traffic)
+        unsigned cta, tid;
+        asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(cta));
+        asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid));
+        const int64_t b2 = (int64_t)cta * kThreads + tid;
+        const int64_t idx = b2 < B ? b2 : B - 1;
         if (!FUSED_BWD || P) store_matrix(P + 16 * idx, out);
         if constexpr (FUSED_BWD) {
             float g[16], d[16];
