@@ -52,14 +52,16 @@ typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
  * Forward projection (section 3).  H, P: device, fp32 [B][4][4].
  *   tol       stop when the marginal error Err(T) = ||T1-1||_1 + ||T^T1-1||_1 of the
  *             current iterate is <= tol.  Rows of T are normalised by construction (eq. (10)), so the
- *             kernel tests the column part |g1|+|g2|+|g3|+|g1+g2+g3|, g = c - 1 (eq. (11)), in fp32
- *             against an internal threshold min(tol, max(tol/2, tol - 5e-7)) that leaves room for the
- *             fp32 rounding of the rows (S3/S9).  tol = 0 runs to the fp32 floor.
+ *             kernel tests the column part |g1|+|g2|+|g3|+|g4|, g = c - 1 (eq. (11)), in fp32
+ *             against an internal threshold max(tol/2, tol - 7e-7) that leaves room for the fp32
+ *             rounding of the stored entries (S3/S9).  tol = 0 runs to the fp32 floor.
  *   max_iter  maximum number of updates of beta per matrix (Newton steps plus, in the guarded solver,
  *             fallback column steps; PAPER.md:319 uses 20).  The start-up steps (three Sinkhorn sweeps
  *             for well-scaled logits, one balancing step after the LP start otherwise; S1) are
- *             not counted: function evaluations <= max_iter + 4.  The first min(2, max_iter) updates
- *             are taken without testing the residual, so a matrix reports at least that many updates.
+ *             not counted: function evaluations <= max_iter + 4.  The first updates are taken without
+ *             testing the residual: min(2, max_iter) for a matrix that starts from beta = 0, 3 for one
+ *             that takes the LP start (if max_iter >= 3), so a matrix reports at least that many; the
+ *             count is a property of the matrix, not of the batch it is in (S2).
  *             A matrix that the lean iteration hands to the guarded solver (S2) is solved again
  *             with the updates that are left, and reports the sum.  max_iter = 0 is accepted (start
  *             point only, rows normalised).
@@ -146,7 +148,8 @@ int birkhoff4_sinkhorn(const float* H, float* P, int64_t B, int n_iter, birkhoff
  *   birkhoff4_forward_host           H_host -> P_host
  *   birkhoff4_backward_host          P_host, dP_host -> dH_host
  *   birkhoff4_forward_backward_host  H_host, dP_host -> P_host (nullable), dH_host
- *                                    (P stays on the device between the two kernels)
+ *                                    (one fused kernel per chunk: P goes from the projection to its
+ *                                    derivative in registers)
  * The ring belongs to the device that is current when it is first used (a call under another current
  * device rebuilds it); calls are serialised by a mutex.  On an error the call still waits for every copy
  * it has started, so no transfer into the caller's buffers is in flight when it returns.
