@@ -243,11 +243,14 @@ struct LeanResult {
 //     v, so the last evaluation is every lane's result and T is handed back once.
 // A lane that is not `active` only follows the warp.  `stored` is false for a matrix whose residual stopped falling
 // above the fp32 floor (and for NaN): the guarded solver takes it.
+// MAY_PLAIN3 = false: the caller knows that no lane of the warp is plain3 (no votes are spent on it).
+template <bool MAY_PLAIN3>
 BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, bool plain3, float tol_i,
                                 int max_iter, float (&T)[16]) {
     float g[4];
     int it = 0;  // this lane's update count
-    const bool any3 = __any_sync(0xffffffffu, plain3), all3 = __all_sync(0xffffffffu, plain3 || !active);
+    const bool any3 = MAY_PLAIN3 && __any_sync(0xffffffffu, plain3);
+    const bool all3 = MAY_PLAIN3 && any3 && __all_sync(0xffffffffu, plain3 || !active);
     if (any3 && all3) {
 #pragma unroll 1
         for (; it < kLeanFreeWide; ++it) {

@@ -39,14 +39,16 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
         const bool finite = valid && spread <= 3.0e38f;  // an infinite (or inf - inf = NaN) range is the guarded solver's
         bool narrow = finite && spread <= lp_range;
         float E[16], T[16], v0, v1, v2;
-        if (__any_sync(0xffffffffu, narrow)) {
+        bool any_narrow = __any_sync(0xffffffffu, narrow);
+        if (any_narrow) {
             float s0[4];
             const float smax = narrow_exponentials(h, rmax, E, s0);
             narrow = narrow && !(smax < kPeakedSum);
-            if (__any_sync(0xffffffffu, narrow)) narrow_sweeps(E, s0, v0, v1, v2);
+            any_narrow = __any_sync(0xffffffffu, narrow);
+            if (any_narrow) narrow_sweeps(E, s0, v0, v1, v2);
         }
         const bool wide = finite && !narrow, active = finite;
-        const bool any_narrow = __any_sync(0xffffffffu, narrow), any_wide = __any_sync(0xffffffffu, wide);
+        const bool any_wide = __any_sync(0xffffffffu, wide);
         if (any_narrow || any_wide) {
             LeanResult res;
             if (any_wide) {
@@ -61,14 +63,14 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
                 } else {
                     code = kIdentityCode;
                 }
-                res = lean_iterate(E, v0, v1, v2, active, wide && max_iter >= kLeanFreeWide, tol_i, max_iter, T);
+                res = lean_iterate<true>(E, v0, v1, v2, active, wide && max_iter >= kLeanFreeWide, tol_i, max_iter, T);
                 if (active && res.stored) {
                     float out[16];
                     unpermute_columns(T, code, sm, out);
                     commit(out);
                 }
             } else {
-                res = lean_iterate(E, v0, v1, v2, active, false, tol_i, max_iter, T);
+                res = lean_iterate<false>(E, v0, v1, v2, active, false, tol_i, max_iter, T);
                 if (active && res.stored) commit(T);
             }
             if (active && res.stored) record(res.it, res.converged);
