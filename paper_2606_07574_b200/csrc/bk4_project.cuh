@@ -66,12 +66,16 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
                 res = lean_iterate<true>(E, v0, v1, v2, active, wide && max_iter >= kLeanFreeWide, tol_i, max_iter, T);
                 if (active && res.stored) {
                     float out[16];
+                    clamp_diagonal(T);
                     unpermute_columns(T, code, sm, out);
                     commit(out);
                 }
             } else {
                 res = lean_iterate<false>(E, v0, v1, v2, active, false, tol_i, max_iter, T);
-                if (active && res.stored) commit(T);
+                if (active && res.stored) {
+                    clamp_diagonal(T);
+                    commit(T);
+                }
             }
             if (active && res.stored) record(res.it, res.converged);
             left = valid && !(active && res.stored);
@@ -100,8 +104,11 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
                 gather_columns(sm, code, Hr);
             };
             auto emit = [&](const float(&T)[16], int iters, bool converged) {
-                float out[16];
-                unpermute_columns(T, code, sm, out);
+                float Tc[16], out[16];
+#pragma unroll
+                for (int q = 0; q < 16; ++q) Tc[q] = T[q];
+                clamp_diagonal(Tc);
+                unpermute_columns(Tc, code, sm, out);
 #pragma unroll
                 for (int q = 0; q < 16; ++q) out[q] = bad ? kNaN : out[q];
                 commit(out);

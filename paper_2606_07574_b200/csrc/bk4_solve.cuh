@@ -86,8 +86,7 @@ BK4_DEV void eval_T(const float (&E)[16], float v0, float v1, float v2, float (&
         T[4 * i + b] = x[b] * r;
         T[4 * i + c] = x[c] * r;
         out[i] = off * r;
-        // (REFINE: an entry of the result.  A diagonal entry below 2^-24 would come out as +-2^-25 of rounding.)
-        T[5 * i] = REFINE ? fmaxf(1.0f - out[i], 0.0f) : 1.0f - out[i];
+        T[5 * i] = 1.0f - out[i];  // (may come out as -2^-25 of rounding when the entry is below 2^-24: clamp_diagonal)
     }
 #pragma unroll
     for (int m = 0; m < (ALL4 ? 4 : 3); ++m) {
@@ -95,6 +94,12 @@ BK4_DEV void eval_T(const float (&E)[16], float v0, float v1, float v2, float (&
         g[m] = ((T[4 * a + m] + T[4 * b + m]) + T[4 * c + m]) - out[m];
     }
     if constexpr (!ALL4) g[3] = 0.0f;
+}
+
+// An evaluation that becomes the result: its diagonal entries 1 - out_m are not allowed below zero.
+BK4_DEV void clamp_diagonal(float (&T)[16]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) T[5 * i] = fmaxf(T[5 * i], 0.0f);
 }
 
 // eval_T<true, false> for the lanes with `refine`, eval_T<false> for the others, bit for bit, in one instruction stream
@@ -114,8 +119,7 @@ BK4_DEV void eval_T_sel(const float (&E)[16], float v0, float v1, float v2, bool
         T[4 * i + b] = x[b] * r;
         T[4 * i + c] = x[c] * r;
         out[i] = off * r;
-        const float diag = 1.0f - out[i];
-        T[5 * i] = refine ? fmaxf(diag, 0.0f) : diag;
+        T[5 * i] = 1.0f - out[i];
     }
 #pragma unroll
     for (int mcol = 0; mcol < 3; ++mcol) {
