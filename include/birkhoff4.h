@@ -55,8 +55,9 @@ typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
  *             kernel tests the column part |g1|+|g2|+|g3|+|g4|, g = c - 1 (eq. (11)), in fp32
  *             against an internal threshold max(tol/2, tol - 7e-7) that leaves room for the fp32
  *             rounding of the stored entries (S3/S9).  tol = 0 runs to the fp32 floor.
- *   max_iter  maximum number of updates of beta per matrix (Newton steps plus, in the guarded solver,
- *             fallback column steps; PAPER.md:319 uses 20).  The start-up steps (three Sinkhorn sweeps
+ *   max_iter  maximum number of updates of beta per matrix (Newton steps, the one Sinkhorn column step
+ *             a nearly converged well-scaled matrix may take instead, and the guarded solver's fallback
+ *             column steps; PAPER.md:319 uses 20).  The start-up steps (three Sinkhorn sweeps
  *             for well-scaled logits, one balancing step after the LP start otherwise; S1) are
  *             not counted: function evaluations <= max_iter + 4.  The first updates are taken without
  *             testing the residual: min(2, max_iter) for a matrix that starts from beta = 0, 3 for one

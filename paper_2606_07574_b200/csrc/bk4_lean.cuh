@@ -19,6 +19,7 @@
 #pragma once
 #include "bk4_solve.cuh"
 
+
 namespace bk4 {
 
 #ifndef BK4_THREADS
@@ -31,6 +32,7 @@ constexpr int kLeanFree = 2;            // Newton updates taken before the first
 constexpr int kLeanFreeWide = 3;        // the same when every matrix of the warp took the wide start
 static_assert(kLeanFree == 2, "lean_iterate spells the free updates out");
 constexpr float kPeakedSum = 1.05f;     // every row sum of exp(H - rowmax) below this: wide start (see narrow_exponentials)
+constexpr float kPolish = 1.5f;          // a residual within this factor of tol_i at the first test: polishing step (lean_iterate)
 constexpr int kLeanNoisy = 4;            // tested updates during which a residual within 4 tol_i may rise
 constexpr float kBalanceFloor = 3e-6f;  // floor of the flows in the balancing step after the LP start
 constexpr unsigned kIdentityCode = 0x03020100u;  // column code: byte m = original column of permuted column m
@@ -243,14 +245,18 @@ struct LeanResult {
 //     v, so the last evaluation is every lane's result and T is handed back once.
 // A lane that is not `active` only follows the warp.  `stored` is false for a matrix whose residual stopped falling
 // above the fp32 floor (and for NaN): the guarded solver takes it.
-// MAY_PLAIN3 = false: the caller knows that no lane of the warp is plain3 (no votes are spent on it).
-template <bool MAY_PLAIN3>
-BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, bool plain3, float tol_i,
-                                int max_iter, float (&T)[16]) {
+// KIND: what the caller knows about the warp (no votes are spent on it, and a warp of wide matrices carries none of
+// the narrow matrices' polishing step): kLeanNarrow = no wide matrix, kLeanWide = no narrow matrix (plain3 is then the
+// same for every lane), kLeanMixed = both.
+constexpr int kLeanNarrow = 0, kLeanMixed = 1, kLeanWide = 2;
+template <int KIND>
+BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float v2, bool active, bool plain3, bool polishable,
+                                float tol_i, int max_iter, float (&T)[16]) {
     float g[4];
     int it = 0;  // this lane's update count
-    const bool any3 = MAY_PLAIN3 && __any_sync(0xffffffffu, plain3);
-    const bool all3 = MAY_PLAIN3 && any3 && __all_sync(0xffffffffu, plain3 || !active);
+    const bool wide3 = KIND == kLeanWide && max_iter >= kLeanFreeWide;  // a warp of wide matrices: nothing to vote on
+    const bool any3 = KIND == kLeanWide ? wide3 : KIND == kLeanMixed && __any_sync(0xffffffffu, plain3);
+    const bool all3 = KIND == kLeanWide ? wide3 : KIND == kLeanMixed && any3 && __all_sync(0xffffffffu, plain3 || !active);
     if (any3 && all3) {
 #pragma unroll 1
         for (; it < kLeanFreeWide; ++it) {
@@ -301,7 +307,30 @@ BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float 
             res.stored = conv || ((it >= max_iter || errprev < kLeanFloor) && err < kInf);  // never a NaN
         }
         if (!__any_sync(0xffffffffu, go)) break;
-        lean_update<true>(T, g, go, v0, v1, v2);
+        // The polishing step.  After the two untested updates a well-scaled matrix that fails its first test is as good
+        // as converged: what is left is the fp32 error of the evaluation the second update started from (measured on
+        // N(0,1): 82 % of them are within 2 tol_i).  Such a matrix (narrow start, in-row range at
+        // most kPolishSpread, residual within kPolish tol_i) takes a Sinkhorn column step from the residuals at hand,
+        // v_m *= c_4 / c_m = 1 + (g_4 - g_m) + O(g^2) (eq. (6) PAPER.md:108 with the gauge v_4 = 1), instead of a Newton
+        // update; a warp in which no other matrix needs one skips the Hessian solve.  The choice is the matrix's own,
+        // it is made once (a matrix that is still not there afterwards takes Newton updates), and it counts as an update.
+        bool cheap = false, polish = false;
+        if (KIND != kLeanWide) {
+            cheap = go && polishable && it == kLeanFree && err <= kPolish * tol_i;
+            polish = __any_sync(0xffffffffu, cheap);
+        }
+        if (!polish) {
+            lean_update<true>(T, g, go, v0, v1, v2);
+        } else {
+            float f0 = 1.0f, f1 = 1.0f, f2 = 1.0f;
+            if (__any_sync(0xffffffffu, go && !cheap)) {
+                float d1, d2, d3;
+                newton_direction<true>(T, g[0], g[1], g[2], d1, d2, d3);
+                f0 = exp_step<true>(d1), f1 = exp_step<true>(d2), f2 = exp_step<true>(d3);
+            }
+            if (cheap) f0 = 1.0f + (g[3] - g[0]), f1 = 1.0f + (g[3] - g[1]), f2 = 1.0f + (g[3] - g[2]);
+            if (go) v0 *= f0, v1 *= f1, v2 *= f2;
+        }
         errprev = go ? err : -1.0f;
     }
     return res;

@@ -6,11 +6,15 @@
 #include "bk4_guarded.cuh"
 #include "bk4_lean.cuh"
 
+
 namespace bk4 {
 
 // largest in-row logit range max_i (max_j H_ij - min_j H_ij) up to which a matrix starts from beta = 0 (above: LP
 // dual start); chosen by measurement, S1.  Row offsets do not matter: eq. (10) removes them.
 constexpr float kLpRange = 12.0f;
+// largest in-row range up to which a narrow matrix may take the polishing step of lean_iterate (beyond, a Sinkhorn step
+// is too weak to be worth the attempt: measured)
+constexpr float kPolishSpread = 5.0f;
 
 // All 32 lanes of a warp must call this together (it votes).  `valid`: this lane holds a matrix.
 //   load(h)              fills h[16] with the lane's logits (called once, and again if the guarded solver is needed)
@@ -49,6 +53,7 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
         }
         const bool wide = finite && !narrow, active = finite;
         const bool any_wide = __any_sync(0xffffffffu, wide);
+        const bool polishable = narrow && spread <= kPolishSpread;  // see lean_iterate
         if (any_narrow || any_wide) {
             LeanResult res;
             if (any_wide) {
@@ -63,7 +68,9 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
                 } else {
                     code = kIdentityCode;
                 }
-                res = lean_iterate<true>(E, v0, v1, v2, active, wide && max_iter >= kLeanFreeWide, tol_i, max_iter, T);
+                const bool plain3 = wide && max_iter >= kLeanFreeWide;
+                res = any_narrow ? lean_iterate<kLeanMixed>(E, v0, v1, v2, active, plain3, polishable, tol_i, max_iter, T)
+                                 : lean_iterate<kLeanWide>(E, v0, v1, v2, active, plain3, false, tol_i, max_iter, T);
                 if (active && res.stored) {
                     float out[16];
                     clamp_diagonal(T);
@@ -71,7 +78,7 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
                     commit(out);
                 }
             } else {
-                res = lean_iterate<false>(E, v0, v1, v2, active, false, tol_i, max_iter, T);
+                res = lean_iterate<kLeanNarrow>(E, v0, v1, v2, active, false, polishable, tol_i, max_iter, T);
                 if (active && res.stored) {
                     clamp_diagonal(T);
                     commit(T);

@@ -345,7 +345,7 @@ def test_lean_iteration_counts_and_floor():
     it = torch.zeros(1 << 14, dtype=torch.int32, device="cuda")
     unc = torch.zeros(1, dtype=torch.int64, device="cuda")
     P = bk.birkhoff4_forward_ex(H, iters=it, n_unconverged=unc)
-    assert int(it.min()) == 2 and int(it.max()) <= 4 and int(unc.item()) == 0
+    assert int(it.min()) == 2 and int(it.max()) <= 5 and int(unc.item()) == 0    # (5: a polishing step that did not do, then Newton updates)
     assert float(it.float().mean()) < 2.1
     it1 = torch.zeros_like(it)
     P1 = bk.birkhoff4_forward_ex(H, max_iter=1, iters=it1)
