@@ -58,15 +58,19 @@ BK4_DEV void project_one(Load&& load, bool valid, float* sm, float tol_i, int ma
             LeanResult res;
             if (any_wide) {
                 // the wide start works on column-permuted matrices: a narrow matrix in the same warp keeps its order
-                float Ew[16], w0, w1, w2;
                 unsigned code;
-                wide_start(h, sm, Ew, w0, w1, w2, code);
-                if (wide || !any_narrow) {
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) E[q] = Ew[q];
-                    v0 = w0, v1 = w1, v2 = w2;
+                if (!any_narrow) {
+                    wide_start(h, sm, E, v0, v1, v2, code);  // straight into E: a warp of wide matrices moves no registers
                 } else {
-                    code = kIdentityCode;
+                    float Ew[16], w0, w1, w2;
+                    wide_start(h, sm, Ew, w0, w1, w2, code);
+                    if (wide) {
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) E[q] = Ew[q];
+                        v0 = w0, v1 = w1, v2 = w2;
+                    } else {
+                        code = kIdentityCode;
+                    }
                 }
                 const bool plain3 = wide && max_iter >= kLeanFreeWide;
                 res = any_narrow ? lean_iterate<kLeanMixed>(E, v0, v1, v2, active, plain3, polishable, tol_i, max_iter, T)
