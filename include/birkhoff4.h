@@ -42,9 +42,11 @@ extern "C" {
 
 #define BIRKHOFF4_OK 0
 #define BIRKHOFF4_EINVAL 1
+#define BIRKHOFF4_ETOOBIG 2 /* birkhoff4_forward_host_static only: B > BIRKHOFF4_STATIC_MAX */
 #define BIRKHOFF4_ECUDA_BASE 1000 /* return value = BIRKHOFF4_ECUDA_BASE + cudaError_t */
 
 #define BIRKHOFF4_HIST_BINS 64
+#define BIRKHOFF4_STATIC_MAX 65536 /* matrices per call of birkhoff4_forward_host_static (4 MiB of device memory) */
 
 typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
 
@@ -160,6 +162,46 @@ int birkhoff4_backward_host(const float* P_host, const float* dP_host, float* dH
 int birkhoff4_forward_backward_host(const float* H_host, const float* dP_host, float* P_host, float* dH_host,
                                     int64_t B, float tol, int max_iter);
 void birkhoff4_host_release(void);
+
+/*
+ * birkhoff4_forward_host for callers that must not allocate device memory: H_host -> P_host, the same forward
+ * kernel and the same results as birkhoff4_forward / birkhoff4_forward_host, but no cudaMalloc, cudaFree, stream
+ * creation or other allocating call is ever made, on the first call or on a later one.
+ *
+ * Who needs it.  birkhoff4_forward_host keeps its device copy of the batch in buffers it gets from cudaMalloc on
+ * first use.  That is unusable when the process has already handed all of the GPU's memory to a pool of its own
+ * (a serving engine that sizes its KV cache to what is free, a training job whose caching allocator has grown to
+ * the card): cudaMalloc then fails although the job itself is far from full.  It is also unusable where a
+ * device-wide stall is not acceptable (cudaMalloc and cudaFree may synchronise the whole device), and in a process
+ * where another thread is recording a CUDA graph in the default (global) capture mode, during which cudaMalloc
+ * from any thread is an error.
+ *
+ * How.  The device copy lives in a fixed array inside the library: BIRKHOFF4_STATIC_MAX matrices, 4 MiB, which
+ * every GPU that loads libbirkhoff4.so holds from the moment the library's code is loaded on it until the process
+ * exits, whether or not this call is ever made.  The logits are copied into it, projected in place and copied
+ * out, all on `stream` (the caller's; 0 = the legacy default stream), and the call returns after waiting for
+ * `stream`, when P_host holds the result.  P_host == H_host is allowed.  Pinned host memory is recommended;
+ * pageable memory works.
+ *
+ *   B > BIRKHOFF4_STATIC_MAX   returns BIRKHOFF4_ETOOBIG (nothing is copied or launched; birkhoff4_strerror names
+ *                              the limit).  Split the batch into several calls, or use birkhoff4_forward_host.
+ *   first call on a device     looks up the array's address on the device that is current (once per device, under a
+ *                              lock; the address is kept).  This may make the driver load the library's device
+ *                              code, so make one call (B = 1 will do) on each device you will use before you begin
+ *                              any stream capture there.
+ *   one array per device       every call on a device uses the same array, from every thread and every stream.  The
+ *                              library does NOT serialise them: two calls whose work overlaps on the GPU (two
+ *                              host threads, hence two calls in flight at once) overwrite each other's matrices.
+ *                              Issue the calls for one device from one thread, or put your own lock around them.
+ *                              Each process has its own copy, so separate processes do not interfere.
+ *   stale contents             the array keeps whatever the last call left in it.  No call depends on that: the
+ *                              first B matrices are overwritten before the kernel reads them and no others are
+ *                              touched, so nothing needs clearing between calls.
+ * Other errors as for birkhoff4_forward (BIRKHOFF4_EINVAL for a null pointer with B > 0, B < 0, bad tol or
+ * max_iter; BIRKHOFF4_ECUDA_BASE + cudaError_t for a failed copy or launch).  B == 0 is a successful no-op.
+ */
+int birkhoff4_forward_host_static(const float* H_host, float* P_host, int64_t B, float tol, int max_iter,
+                                  birkhoff4_stream_t stream);
 
 const char* birkhoff4_strerror(int code);
 int birkhoff4_version(void);

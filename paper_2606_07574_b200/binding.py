@@ -17,6 +17,7 @@ import torch
 from . import build as _build
 
 HIST_BINS = 64
+STATIC_MAX = 65536      # BIRKHOFF4_STATIC_MAX: matrices per call of birkhoff4_forward_host_static
 _LIB = None
 
 
@@ -47,6 +48,7 @@ def lib():
             "forward_host": [vp, vp, i64, f32, ci],
             "backward_host": [vp, vp, vp, i64],
             "forward_backward_host": [vp, vp, vp, vp, i64, f32, ci],
+            "forward_host_static": [vp, vp, i64, f32, ci, vp],
             "version": [],
         }
         for name, args in sig.items():
@@ -227,6 +229,24 @@ def birkhoff4_forward_host(H_host, P_host=None, tol=1e-6, max_iter=20):
     H_host = _host(H_host, "H_host")
     P_host = torch.empty_like(H_host) if P_host is None else _host(P_host, "P_host", H_host.numel())
     _check(lib().birkhoff4_forward_host(_ptr(H_host), _ptr(P_host), H_host.numel() // 16, tol, max_iter))
+    return P_host
+
+
+def birkhoff4_forward_host_static(H_host, P_host=None, tol=1e-6, max_iter=20, stream=None):
+    """birkhoff4_forward_host without any device allocation, for at most STATIC_MAX (65536) matrices per call.
+
+    For processes in which cudaMalloc is not an option: all GPU memory already belongs to the process's own pool
+    (a serving engine's KV cache, a grown caching allocator), a device-wide stall cannot be afforded, or another
+    thread is capturing a CUDA graph.  The device copy of the batch sits in a 4 MiB array built into the library.
+    CPU tensors in and out (the output is a CPU tensor: no CUDA tensor is created here either), synchronous.
+    Raises Birkhoff4Error for a larger batch.  All calls on one device share that array: do not run two at once
+    from different threads.  Make the first call on a device before any stream capture (include/birkhoff4.h).
+    `stream`: a torch.cuda.Stream, or None for the current device's legacy default stream (0).
+    """
+    H_host = _host(H_host, "H_host")
+    P_host = torch.empty_like(H_host) if P_host is None else _host(P_host, "P_host", H_host.numel())
+    st = ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)
+    _check(lib().birkhoff4_forward_host_static(_ptr(H_host), _ptr(P_host), H_host.numel() // 16, tol, max_iter, st))
     return P_host
 
 

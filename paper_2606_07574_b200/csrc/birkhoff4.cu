@@ -313,6 +313,58 @@ static int launch_mix(const float* H, const void* X, void* Y, float* P, int64_t 
                           internal_tol(tol), max_iter, kLpRange));
 }
 
+// ---- host-buffer forward that allocates nothing (birkhoff4_forward_host_static)
+// The device copy of the batch lives in this array instead of in buffers from cudaMalloc: 4 MiB that every GPU
+// which loads the library holds until the process exits.  The logits are copied in, projected IN PLACE (P == H is
+// an allowed alias of the forward kernel) and copied out, so one region serves as input and output.
+// Nothing here has to start at zero: a call overwrites the first B matrices before the kernel reads them and the
+// kernel touches no others, so what an earlier call left behind is never read.
+static __device__ __align__(256) float g_static_stage[BIRKHOFF4_STATIC_MAX * 16];
+
+// In host code `g_static_stage` is only a handle for the runtime, not an address a kernel can use.  The device
+// address differs from GPU to GPU, so it is asked for once per device, with that device current, and kept.
+struct StaticStage {
+    static constexpr int kMaxDevices = 64;
+    std::mutex mu;
+    float* addr[kMaxDevices] = {};
+};
+static StaticStage g_static;
+
+static int static_stage_address(float** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_rc(e);
+    if (dev < 0 || dev >= StaticStage::kMaxDevices) return BIRKHOFF4_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static.mu);
+    if (!g_static.addr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_stage);  // first use on this device: may load the module (do it before any capture)
+        if (e != cudaSuccess) return cuda_rc(e);
+        if (!p || misaligned(p)) return BIRKHOFF4_EINVAL;
+        g_static.addr[dev] = static_cast<float*>(p);
+    }
+    *out = g_static.addr[dev];
+    return BIRKHOFF4_OK;
+}
+
+static int run_host_static(const float* H_host, float* P_host, int64_t B, float tol, int max_iter, cudaStream_t stream) {
+    if (B < 0 || !(tol >= 0.0f) || max_iter < 0) return BIRKHOFF4_EINVAL;
+    if (B > BIRKHOFF4_STATIC_MAX) return BIRKHOFF4_ETOOBIG;  // before anything touches the device
+    if (B == 0) return BIRKHOFF4_OK;
+    if (!H_host || !P_host) return BIRKHOFF4_EINVAL;
+    float* stage = nullptr;
+    int rc = static_stage_address(&stage);
+    if (rc) return rc;
+    const size_t bytes = (size_t)B * 64;
+    rc = cuda_rc(cudaMemcpyAsync(stage, H_host, bytes, cudaMemcpyHostToDevice, stream));
+    if (!rc) rc = launch_forward<false>(stage, stage, B, tol, max_iter, FwdDiag{nullptr, nullptr, nullptr}, stream);
+    if (!rc) rc = cuda_rc(cudaMemcpyAsync(P_host, stage, bytes, cudaMemcpyDeviceToHost, stream));
+    // also on an error: nothing is still reading or writing the caller's buffers when the call returns
+    const cudaError_t e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess && rc == BIRKHOFF4_OK) rc = cuda_rc(e);
+    return rc;
+}
+
 }  // namespace bk4
 
 // =================================================================== C ABI
@@ -387,6 +439,11 @@ int birkhoff4_forward_backward_host(const float* H_host, const float* dP_host, f
     return run_host(H_host, nullptr, dP_host, P_host, dH_host, B, tol, max_iter, 3);
 }
 
+int birkhoff4_forward_host_static(const float* H_host, float* P_host, int64_t B, float tol, int max_iter,
+                                  birkhoff4_stream_t stream) {
+    return run_host_static(H_host, P_host, B, tol, max_iter, (cudaStream_t)stream);
+}
+
 void birkhoff4_host_release(void) {
     std::lock_guard<std::mutex> lock(g_ring.mu);
     g_ring.teardown();
@@ -395,6 +452,9 @@ void birkhoff4_host_release(void) {
 const char* birkhoff4_strerror(int code) {
     if (code == BIRKHOFF4_OK) return "success";
     if (code == BIRKHOFF4_EINVAL) return "invalid argument (null or misaligned pointer, negative size, bad tol/max_iter)";
+    if (code == BIRKHOFF4_ETOOBIG)
+        return "batch too large for birkhoff4_forward_host_static: at most BIRKHOFF4_STATIC_MAX (65536) matrices per call; "
+               "split the batch or use birkhoff4_forward_host";
     if (code >= BIRKHOFF4_ECUDA_BASE) return cudaGetErrorString((cudaError_t)(code - BIRKHOFF4_ECUDA_BASE));
     return "unknown error";
 }
