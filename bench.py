@@ -15,8 +15,14 @@ L2: every rank rotates over `sets` distinct buffer sets (H, P, dP, dH; >= 1 GiB 
 runs forward on set i % sets and backward on set (i+1) % sets, whose P was written sets-1 steps earlier, so
 backward reads P from HBM as it does in training, where the rest of the network runs in between.
 
-One JSON line on stdout (rank 0).  `value` = matrices/s through forward+backward with inputs resident in HBM
-(K steps between two CUDA events on the launching stream, max over ranks); `e2e` = the same through the
+ONE compact JSON line on stdout (rank 0; contract_line(), under 2 KB: the driver keeps a bounded tail of stdout).
+The full result (every other BASELINE.json config under `workloads`, the SURVEY.md 8(f) widenings, histograms)
+goes to gpurun_out/bench_detail.json and, as one line, to stderr; `per_config` in the stdout line carries
+[step us, forward frac, backward frac, max Err] of each other config.
+`value` = matrices/s through forward+backward with inputs resident in HBM: the median over --regions regions of K
+steps each between two CUDA events on the launching stream (max over ranks); `value_single` = the one K-step region
+bracketed by barrier + synchronize; `roofline.isolated_us` = the forward launched alone after an L2-displacing
+write (no overlap with a neighbouring launch), `roofline.avg_us` = back to back; `e2e` = the same through the
 host-buffer C-ABI call birkhoff4_forward_backward_host (pinned host memory in, P and dH back out, copies inside
 the timed region); `roofline_kernels` = each kernel's average launch duration (K back-to-back launches of that
 kernel over the same rotation between two events) against the measured HBM copy bandwidth (MEASURED_PEAKS.json),
@@ -149,6 +155,76 @@ def _finite(x):
     return x
 
 
+# ------------------------------------------------------------------------------------------------ the contract line
+LINE_LIMIT = 2048       # bytes: the driver keeps a bounded tail of stdout, so the one JSON line must stay small
+
+
+def _r(x, nd=4):
+    """numbers rounded to `nd` significant digits (the detail file keeps full precision)"""
+    if isinstance(x, float):
+        return float("%.*g" % (nd, x)) if np.isfinite(x) else None
+    if isinstance(x, dict):
+        return {k: _r(v, nd) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_r(v, nd) for v in x]
+    return x
+
+
+def contract_line(full):
+    """the ONE stdout line: the contract keys of the full result only, under LINE_LIMIT bytes.  Everything else
+    (per-workload blocks, widenings, histograms) goes to the detail file and to stderr."""
+    rf = full["roofline"]
+    line = {k: full[k] for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                                 "scaling", "vs_baseline", "dtype", "data")}
+    line["value_single"] = full.get("value_single")
+    c = full["config"]
+    line["config"] = {k: c[k] for k in ("workload", "desc", "B_per_gpu", "tol", "max_iter", "l2") if k in c}
+    line["roofline"] = {k: rf.get(k) for k in ("kernel", "bound", "achieved", "peak", "unit", "frac", "avg_us", "isolated_us",
+                                               "frac_isolated", "bytes_per_launch", "traffic", "peak_source")}
+    line["roofline_step"] = {k: full["roofline_step"].get(k) for k in ("bound", "achieved", "peak", "unit", "frac")}
+    line["fwd_us"], line["bwd_us"] = full["fwd"]["us"]["median"], full["bwd"]["us"]["median"]
+    line["bwd_frac"] = full["roofline_kernels"]["backward_kernel"]["frac"]
+    line["max_marginal_err"] = full["max_marginal_err"]
+    line["mean_newton_updates"] = full["fwd"]["mean_newton_updates"]
+    if full.get("cpu_baseline"):
+        line["cpu_baseline"] = {k: full["cpu_baseline"][k] for k in ("value", "unit", "cores", "kind", "sample")}
+    e = full["e2e"]
+    line["e2e"] = {k: e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps", "api")}
+    line["clocks"] = full.get("clocks")
+    line["gpu_launches"] = full.get("gpu_launches")
+    if full.get("workloads"):
+        # name: [step_us, forward frac of HBM peak, backward frac, max marginal error]
+        line["per_config"] = {n: [w["step_us"]["median"], w["roofline_kernels"]["forward_kernel"]["frac"],
+                                  w["roofline_kernels"]["backward_kernel"]["frac"], w["max_marginal_err"]]
+                              for n, w in full["workloads"].items() if "@" not in n}
+    if full.get("detail_file"):
+        line["detail_file"] = full["detail_file"]
+    line = _r(_finite(line))
+    text = json.dumps(line, separators=(",", ":"))
+    if len(text) > LINE_LIMIT:                                                 # never the case today; keep the contract keys
+        for k in ("per_config", "detail_file", "roofline_step", "value_single"):
+            line.pop(k, None)
+        text = json.dumps(line, separators=(",", ":"))
+    return text
+
+
+def write_detail(full):
+    """the full result: gpurun_out/bench_detail.json when that folder can be written, and one line on stderr"""
+    text = json.dumps(_finite(full))
+    path = None
+    try:
+        d = os.path.join(ROOT, "gpurun_out")
+        os.makedirs(d, exist_ok=True)
+        path = os.path.join(d, "bench_detail.json")
+        with open(path, "w") as f:
+            f.write(text + "\n")
+        path = os.path.relpath(path, ROOT)
+    except OSError:
+        path = None
+    print(text, file=sys.stderr)
+    return path
+
+
 # ------------------------------------------------------------------------------------------------ reference arm
 def oracle_step(oracle, H, G, nthreads=0):
     P = oracle.forward(H, nthreads=nthreads)
@@ -207,7 +283,7 @@ def _rooflines(B, bf16, f_us, b_us, s_us, peak, peak_src, workload, mean_updates
     if winst:
         issue_peak = 4.0 * n_sm * sm_mhz * 1e6                                 # warp instructions / s
         ach_i = winst * (B / 32.0) / (f_us["median"] * 1e-6)
-        k["forward_kernel"]["alu"] = {
+        k["forward_kernel"]["issue_diagnostic"] = {
             "bound": "alu", "achieved": ach_i / 1e12, "peak": issue_peak / 1e12, "unit": "T warp-instr/s", "frac": ach_i / issue_peak,
             "warp_instr_per_32_matrices": winst, "source": "ncu smsp__inst_executed.sum of this workload (profiles/traffic.csv)",
             "peak_source": "nominal: 4 issue slots per clock per SM x %d SMs x %d MHz (half-rate instructions hold a slot for "
@@ -258,6 +334,23 @@ class Timer:
             e1.synchronize()
             per.append(e0.elapsed_time(e1) * 1e3 / self.K)
         return {"median": statistics.median(per), "min": min(per), "regions": self.R, "calls_per_region": self.K}
+
+
+def isolated_us(torch, fn, n=20):
+    """one launch alone between two events, after a 256 MiB write has displaced L2 (126 MB): median us over n.
+    No back-to-back overlap (programmatic dependent launch) helps this figure; it includes the launch's own ramp and tail."""
+    flush = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+    per = []
+    for i in range(n):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn(i)
+        e1.record()
+        e1.synchronize()
+        per.append(e0.elapsed_time(e1) * 1e3)
+    del flush
+    return statistics.median(per)
 
 
 def err_stats(torch, P):
@@ -313,6 +406,7 @@ def measure_workload(torch, bk, inputs, name, wl, rank, K, R, peak, peak_src, sm
     torch.cuda.synchronize()
     timer = Timer(torch, K, R)
     s_us, f_us, b_us = timer(step), timer(f_call), timer(b_call)
+    f_iso = isolated_us(torch, f_call)
     acc = err_stats(torch, sets[0]["P"])
     hist = torch.zeros(64, dtype=torch.int64, device="cuda")
     unc = torch.zeros(1, dtype=torch.int64, device="cuda")
@@ -321,6 +415,8 @@ def measure_workload(torch, bk, inputs, name, wl, rank, K, R, peak, peak_src, sm
     h = hist.cpu().numpy()
     mean_updates = float((h * np.arange(64)).sum() / max(h.sum(), 1))
     kern, step_roof = _rooflines(B, bf16, f_us, b_us, s_us, peak, peak_src, name, mean_updates, sm_mhz, n_sm)
+    kern["forward_kernel"]["isolated_us"] = f_iso
+    kern["forward_kernel"]["frac_isolated"] = B * (96 if bf16 else FWD_BYTES) / (f_iso * 1e-6) / 1e9 / peak
     res = {"desc": wl["desc"] + (", sorted by class" if sort_by_class else ""), "B": B, "max_iter": max_iter,
            "value": B / (s_us["median"] * 1e-6), "unit": UNIT, "step_us": s_us, "forward_us": f_us, "backward_us": b_us,
            "fwd_matrices_per_s": B / (f_us["median"] * 1e-6), "roofline_step": step_roof, "roofline_kernels": kern,
@@ -438,7 +534,11 @@ def run_ours(args, wl):
     clocks.sample()
     barrier()
     total_ms = shard.reduce_max_time(ev[0].elapsed_time(ev[1]), dist if world > 1 else None)
-    value = world * B * K / (total_ms * 1e-3)
+    value_single = world * B * K / (total_ms * 1e-3)                           # this one region of K steps
+    # `value`: the median over the R regions of K steps each (max over ranks of the per-rank median); one region of
+    # K = 20 steps is a 1 ms sample
+    med_ms = shard.reduce_max_time(head["step_us"]["median"] * 1e-3, dist if world > 1 else None)
+    value = world * B / (med_ms * 1e-3)
 
     # ---- Sinkhorn-20 baseline kernel of the same library (context: PAPER.md:32, 319), fp32 workloads only
     sink = None
@@ -468,7 +568,6 @@ def run_ours(args, wl):
     del sets, Hh, Gh, Ph, dHh
     torch.cuda.empty_cache()
 
-    launches = 2 * K
     if rank != 0:
         clocks.stop()
         if world > 1:
@@ -477,7 +576,8 @@ def run_ours(args, wl):
     fk = head["roofline_kernels"]["forward_kernel"]
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
-        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": med_ms, "value_single": value_single, "ms_per_step_single": total_ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "desc": wl["desc"], "B_per_gpu": B, "tol": TOL, "max_iter": max_iter,
                    "parallelism": "batch shards, no collective" if world > 1 else "single GPU",
@@ -505,7 +605,6 @@ def run_ours(args, wl):
             base = name.split("@")[0]
             res, s_, _ = measure_workload(torch, bk, inputs, base, WORKLOADS[base], 0, Kx, Rx, peak, peak_src, sm_mhz,
                                           props.multi_processor_count, **kw)
-            launches += 3 * Kx * Rx
             extra[name] = res
             del s_
             torch.cuda.empty_cache()
@@ -513,8 +612,7 @@ def run_ours(args, wl):
         out["widenings"] = measure_widenings(torch, bk, inputs, Kx, min(Rx, 5), peak)
         clocks.region(False)
     clocks.stop()
-    out["gpu_launches"] = launches
-    out["gpu_launches_timed_region"] = 2 * K
+    out["gpu_launches"] = 2 * K                                               # per timed region of K steps: forward + backward kernel
     out["clocks"] = clocks.summary()
     if world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -531,7 +629,9 @@ def run_ours(args, wl):
                                "sample": "first %d matrices of buffer set 0, forward+backward, fp64, %.1f s" % (n, dt),
                                "one_thread": {"value": n1 / dt1, "unit": UNIT, "cores": 1,
                                               "sample": "first %d matrices, %.1f s" % (n1, dt1)}}
-    print(json.dumps(_finite(out)))
+    out["detail_file"] = write_detail(out)
+    sys.stderr.flush()
+    print(contract_line(out), flush=True)                                      # the last (and only) stdout line
     if world > 1:
         dist.destroy_process_group()
 

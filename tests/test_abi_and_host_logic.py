@@ -170,3 +170,65 @@ def test_bench_reference_arm_runs_on_cpu():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "matrices/s"
+    assert len(out.stdout.strip().splitlines()[-1]) < 2048
+
+
+def _canned_bench_result():
+    """a full bench result of the shape run_ours() builds, with made-up numbers (no GPU): what contract_line() is fed"""
+    us = {"median": 28.123456789, "min": 27.987654321, "regions": 10, "calls_per_region": 20}
+    kern = lambda frac: {"bound": "hbm", "achieved": 4673.123456, "peak": 6556.8, "unit": "GB/s", "frac": frac,   # noqa: E731
+                         "frac_min_time": 0.72, "frac_of_nominal_7700": 0.61, "avg_us": 28.123456789, "min_us": 27.9,
+                         "bytes_per_launch": 134217728, "traffic": 91435776.0, "isolated_us": 31.4, "frac_isolated": 0.652,
+                         "issue_diagnostic": {"bound": "alu", "frac": 0.5, "peak_source": "x" * 300}}
+    wl = {"desc": "B=2^20 fp32, H iid N(0,10^2)", "step_us": us, "forward_us": us, "backward_us": us, "max_marginal_err": 9.6e-7,
+          "roofline_kernels": {"forward_kernel": kern(0.48), "backward_kernel": kern(1.01)},
+          "update_histogram": {str(k): 0.01 for k in range(40)}}
+    names = ["config3_s10", "config3_s10@max_iter20", "config3_s30", "config3_s30@max_iter20", "config3_s100",
+             "config3_s100@max_iter20", "config4", "config5", "config5@sorted_by_class"]
+    return {
+        "metric": "4x4 projections/sec fwd+bwd", "value": 1.8234567891e10, "unit": "matrices/s", "n_gpus": 1, "steps": 20,
+        "warmup": 5, "ms_per_step": 0.0573123456, "value_single": 1.81e10, "ms_per_step_single": 0.0579,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config2", "desc": "B=2^20 fp32, H,dP iid N(0,1)", "B_per_gpu": 1 << 20, "tol": 1e-6,
+                   "max_iter": 20, "parallelism": "single GPU",
+                   "l2": "rotation over 5 buffer sets (>= 1 GiB); backward reads the P written 4 steps earlier",
+                   "repeats": "every per-kernel and per-step time is the median (and min) of 10 regions of 20 calls"},
+        "roofline": dict(kern(0.713), kernel="forward_kernel", peak_source="measured (MEASURED_PEAKS.json hbm_gbs)"),
+        "roofline_step": {"bound": "hbm", "achieved": 5855.1, "peak": 6556.8, "unit": "GB/s", "frac": 0.893,
+                          "bytes_per_step": 335544320, "peak_source": "measured (MEASURED_PEAKS.json hbm_gbs)"},
+        "roofline_kernels": {"forward_kernel": kern(0.713), "backward_kernel": kern(1.01)},
+        "fwd": {"value": 3.7e10, "unit": "matrices/s", "us": us, "mean_newton_updates": 2.31,
+                "update_histogram": {"2": 0.7, "3": 0.29, "4": 0.01}, "unconverged": 0},
+        "bwd": {"us": us}, "step_us": us, "max_marginal_err": 9.5e-7, "mean_marginal_err": 2.2e-7, "max_err_inf": 2.4e-7,
+        "sinkhorn20_gpu": {"fwd_matrices_per_s": 4e10, "us": us, "max_marginal_err": float("nan")},
+        "e2e": {"value": 3.18e8, "unit": "matrices/s", "h2d_bytes_per_step": 1 << 27, "d2h_bytes_per_step": 1 << 27, "steps": 20,
+                "api": "birkhoff4_forward_backward_host(H_host, dP_host -> P_host, dH_host), fp32 pinned host buffers"},
+        "workloads": {n: wl for n in names}, "widenings": {"x": {"us": us}},
+        "gpu_launches": 5440, "gpu_launches_timed_region": 40,
+        "clocks": {"sm_mhz": 1965.0, "sm_max_mhz": 1965, "reasons": ["sw_power_cap"], "samples": 812},
+        "cpu_baseline": {"value": 1.1e5, "unit": "matrices/s", "cores": 32, "kind": "oracle",
+                         "sample": "first 1048576 matrices of buffer set 0, forward+backward, fp64, 9.8 s",
+                         "one_thread": {"value": 5e3, "unit": "matrices/s", "cores": 1, "sample": "first 65536 matrices, 12.9 s"}},
+        "detail_file": "gpurun_out/bench_detail.json",
+    }
+
+
+def test_bench_contract_line_is_compact_and_complete():
+    """the one stdout line of bench.py: strict JSON, under 2 KB, every key of the driver's contract present (round 2's
+    26 KB line could not be parsed from the driver's bounded stdout tail)"""
+    import json
+    sys.path.insert(0, ROOT)
+    import bench
+    text = bench.contract_line(_canned_bench_result())
+    assert len(text) < bench.LINE_LIMIT == 2048 and "\n" not in text and "NaN" not in text
+    line = json.loads(text)
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "clocks", "gpu_launches"):
+        assert k in line, k
+    assert line["value"] > 0 and line["config"]["workload"] == "config2"
+    assert {"bound", "achieved", "peak", "unit", "frac", "traffic"} <= set(line["roofline"])
+    assert line["roofline"]["bound"] == "hbm" and abs(line["roofline"]["frac"] - 0.713) < 1e-3
+    assert {"value", "unit", "cores", "kind", "sample"} == set(line["cpu_baseline"])
+    assert {"value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step"} <= set(line["e2e"])
+    assert sorted(line["per_config"]) == ["config3_s10", "config3_s100", "config3_s30", "config4", "config5"]
+    assert len(line["per_config"]["config5"]) == 4
