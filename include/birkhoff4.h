@@ -19,7 +19,9 @@
  *   pointers   DEVICE pointers unless the name ends in _host; owned by the caller.  The library never
  *              allocates or frees device memory in the device-pointer calls and never synchronises:
  *              every call is asynchronous on `stream` (a cudaStream_t; 0 = the legacy default stream).
- *   alignment  every matrix pointer must be 32-byte aligned (else BIRKHOFF4_EINVAL; there is no slow path).
+ *   alignment  every matrix pointer must be 32-byte aligned (else BIRKHOFF4_EINVAL; there is no slow path): a
+ *              thread moves its 64-byte matrix with two 256-bit loads or stores (ld/st.global.v8.f32), which
+ *              need their address aligned to 32 bytes.  (SURVEY.md 8(b) proposed 16, the 128-bit rule.)
  *   aliasing   P == H and dH == dP are allowed as exact aliases; partial overlap is undefined.
  *   errors     return 0 on success; BIRKHOFF4_EINVAL for a null pointer with B > 0, B < 0, tol < 0 or NaN,
  *              max_iter < 0, n_iter < 0 or a misaligned pointer; BIRKHOFF4_ECUDA_BASE + cudaError_t if
@@ -61,7 +63,10 @@ typedef struct CUstream_st* birkhoff4_stream_t; /* identical to cudaStream_t */
  *             a nearly converged well-scaled matrix may take instead, and the guarded solver's fallback
  *             column steps; PAPER.md:319 uses 20).  The start-up steps (three Sinkhorn sweeps
  *             for well-scaled logits, one balancing step after the LP start otherwise; S1) are
- *             not counted: function evaluations <= max_iter + 4.  The first updates are taken without
+ *             not counted: function evaluations <= max_iter + 4 for a matrix the lean iteration finishes.  (One
+ *             it hands to the guarded solver starts again there: the start-up evaluations are spent a second
+ *             time and every rejected trial step costs one more, so only the update count is bounded for it.)
+ *             The first updates are taken without
  *             testing the residual: min(2, max_iter) for a matrix that starts from beta = 0, 3 for one
  *             that takes the LP start (if max_iter >= 3), so a matrix reports at least that many; the
  *             count is a property of the matrix, not of the batch it is in (S2).

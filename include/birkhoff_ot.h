@@ -23,8 +23,10 @@
  *   tol        stop when Err_ab(T) = ||T1 - a||_1 + ||T^T1 - b||_1 (PAPER.md:323 with marginals a, b) <= tol.
  *              Rows equal a by construction, so the kernel tests the column part against tol / 2.  fp32 floor:
  *              about 2.5e-7 per unit of sum(a) / 4 (so 1e-6 is reachable for 4x4 with unit marginals, 2e-6 for 8x8).
- *   max_iter   maximum number of updates of beta (Newton steps and fallback Sinkhorn steps) over all
- *              continuation stages; the three Sinkhorn sweeps that start each stage are not counted.
+ *   max_iter   maximum number of updates of beta over all continuation stages.  An update is a Newton step, a
+ *              retry of a Newton step at half its length (up to four per step, when the step did not lower the
+ *              residual) or a fallback Sinkhorn step; `iters` counts the same.  The three Sinkhorn sweeps that
+ *              start each stage are not counted.
  *   NaN/Inf    a problem holding a NaN or Inf cost gives an all-NaN T for that problem only.
  *   errors     0 on success; BIRKHOFF_OT_EINVAL for bad sizes, a null or misaligned pointer with B > 0, B < 0,
  *              tol < 0 or NaN, max_iter < 0, eta <= 0 or not finite, exactly one of a, b NULL;

@@ -81,7 +81,6 @@ static int forward_dispatch(const float* C, const float* a, const float* b, floa
                             float eta, float tol, int max_iter, int32_t* iters, unsigned long long* unc, cudaStream_t st) {
     if (B < 0 || !(tol >= 0.0f) || max_iter < 0 || !(eta > 0.0f) || !(eta < 3.0e38f)) return BIRKHOFF_OT_EINVAL;
     if ((a == nullptr) != (b == nullptr)) return BIRKHOFF_OT_EINVAL;
-    if (a && n != m && false) return BIRKHOFF_OT_EINVAL;
     if (!a && n != m) return BIRKHOFF_OT_EINVAL;  // unit marginals need a square problem (sum a = sum b)
     if (!((n == 4 || n == 8) && (m == 4 || m == 8))) return BIRKHOFF_OT_EINVAL;
     if (B == 0) return BIRKHOFF_OT_OK;

@@ -304,7 +304,10 @@ BK4_DEV LeanResult lean_iterate(const float (&E)[16], float v0, float v1, float 
         if (errprev >= 0.0f && !go) {  // this lane's matrix is finished
             res.it = it;
             res.converged = conv;
-            res.stored = conv || ((it >= max_iter || errprev < kLeanFloor) && err < kInf);  // never a NaN
+            // (T is the evaluation at hand.  Out of updates: that is the last iterate.  Stalled: the evaluation is the one
+            // at the trial that did not lower the residual, so it is the result only if it, too, is at the fp32 floor;
+            // a trial that threw the residual back up goes to the guarded solver, which returns an accepted point.)
+            res.stored = conv || (it >= max_iter && err < kInf) || (errprev < kLeanFloor && err < kLeanFloor);  // never a NaN
         }
         if (!__any_sync(0xffffffffu, go)) break;
         // The polishing step.  After the two untested updates a well-scaled matrix that fails its first test is as good

@@ -249,6 +249,16 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
         }
         suma += UNIT ? 1.0f : a[i];
     }
+    if (!((hi - lo) < kInf)) {
+        // an Inf among the costs: there is no finite range to build a continuation schedule on (it would run all 24
+        // stages before the NaN came out); the result is the all-NaN matrix the header promises, at once
+        float x[M];
+#pragma unroll
+        for (int j = 0; j < M; ++j) x[j] = kNaN;
+#pragma unroll
+        for (int i = 0; i < N; ++i) store_row<M>(Tg + i * M, x);
+        return OtStats{0, false};
+    }
     const float lam = kOtLam * suma * (1.0f / N);
     float eta_s = eta;
     int stages = 0;
