@@ -27,6 +27,12 @@
  *              retry of a Newton step at half its length (up to four per step, when the step did not lower the
  *              residual) or a fallback Sinkhorn step; `iters` counts the same.  The three Sinkhorn sweeps that
  *              start each stage are not counted.
+ *   regime     costs of any finite range: a range wider than 16 eta is reached by continuation (eta 2^K, ..., 2 eta,
+ *              eta, at most 24 halvings, i.e. range / eta up to 2.7e8), every stage drawing on the same max_iter;
+ *              a problem that runs out of updates on the way is written as it stands (rows equal to a) and counted
+ *              in n_unconverged.  Tested against the oracle for range / eta up to about 1000 (n = 8 logits
+ *              N(0,100^2); costs N(0,3^2) at eta = 0.1) and for marginals down to 1e-6 of the total mass, where 60
+ *              to 80 updates suffice; max_iter = 40 covers range / eta up to about 100.
  *   NaN/Inf    a problem holding a NaN or Inf cost gives an all-NaN T for that problem only.
  *   errors     0 on success; BIRKHOFF_OT_EINVAL for bad sizes, a null or misaligned pointer with B > 0, B < 0,
  *              tol < 0 or NaN, max_iter < 0, eta <= 0 or not finite, exactly one of a, b NULL;

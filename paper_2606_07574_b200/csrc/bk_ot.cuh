@@ -30,6 +30,7 @@ constexpr float kOtLam = 2.384185791015625e-07f;  // ground regularisation, rela
 constexpr int kOtSweeps = 3;                     // Sinkhorn sweeps at the start of every continuation stage
 constexpr float kOtStageRange = 16.0f;           // a stage's scaled costs span at most this (8 / 12 / 16 / 20 / 24 measured: DESIGN.md)
 constexpr int kOtHalvings = 4;                   // step halvings before the Sinkhorn fallback
+constexpr float kOtTiny = 1e-30f;                // floor of a row sum s_i and of a column sum q_j before their reciprocals
 constexpr float kOtStageTol = 1e-2f;             // relative marginal error at which an intermediate stage is left
 
 // vector load/store of one row of K floats (K = 4: 128 bits, K = 8: 256 bits, else scalar)
@@ -162,6 +163,7 @@ BK4_DEV void ot_eval(const float (&E)[N * M], const float (&v)[M - 1], const flo
             x[j] = E[i * M + j] * v[j];
             s += x[j];
         }
+        s = fmaxf(s, kOtTiny);  // a row whose every term underflowed: a finite (huge) residual instead of Inf * 0 = NaN
         float r = rcp_approx(s);
         r = fmaf(r, fmaf(-s, r, 1.0f), r);
         const float ar = UNIT ? r : a[i] * r;
@@ -216,13 +218,17 @@ BK4_DEV void ot_sweep(const float (&E)[N * M], float (&v)[M - 1], const float (&
         float s = E[i * M + M - 1];
 #pragma unroll
         for (int j = 0; j < M - 1; ++j) s = fmaf(E[i * M + j], v[j], s);
+        s = fmaxf(s, kOtTiny);
         const float u = UNIT ? rcp_approx(s) : a[i] * rcp_approx(s);
 #pragma unroll
         for (int j = 0; j < M; ++j) q[j] = fmaf(E[i * M + j], u, q[j]);
     }
-    const float t = UNIT ? q[M - 1] : q[M - 1] * rcp_approx(b[M - 1]);  // 1 / v_M before the gauge
+    // (a column of E that underflowed to zero, e.g. under a tiny b_j late in the continuation, gives q_j = 0: clamped,
+    // so that v_j becomes large and finite instead of Inf and the guard can still judge the step; bk4_guarded.cuh
+    // clamps its column ratios for the same reason)
+    const float t = UNIT ? fmaxf(q[M - 1], kOtTiny) : fmaxf(q[M - 1], kOtTiny) * rcp_approx(b[M - 1]);  // 1 / v_M before the gauge
 #pragma unroll
-    for (int j = 0; j < M - 1; ++j) v[j] = (UNIT ? t : b[j] * t) * rcp_approx(q[j]);
+    for (int j = 0; j < M - 1; ++j) v[j] = (UNIT ? t : b[j] * t) * rcp_approx(fmaxf(q[j], kOtTiny));
 }
 
 struct OtStats {
