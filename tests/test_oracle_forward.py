@@ -180,3 +180,29 @@ def test_empty_and_nonfinite(oracle):
     assert np.isnan(P[1]).all() and np.isnan(P[2]).all()
     assert np.isfinite(P[0]).all() and np.isfinite(P[3]).all()
     assert oracle.marginal_err(P[[0, 3]]).max() < 1e-13
+
+
+def test_marginal_error_helpers_on_hand_built_matrices(oracle):
+    """pins of oracle.marginal_err_inf and oracle.marginal_err on matrices whose row and column
+    deviations are known by construction, not computed by the helpers: T = 1/4 + D with D built from chosen row
+    deviations r and column deviations c (sum r = sum c) as D_ij = r_i/4 + c_j/4 - sum(r)/16, whose row sums are r_i and
+    column sums c_j exactly in exact arithmetic."""
+    r = np.array([3e-7, -1e-7, 0.0, 0.0])
+    c = np.array([2e-7, 0.0, 5e-8, -5e-8])                          # sum r = sum c = 2e-7
+    D = r[:, None] / 4 + c[None, :] / 4 - r.sum() / 16
+    T = (0.25 + D)[None]
+    assert abs(oracle.marginal_err_inf(T)[0] - 3e-7) < 1e-15        # the largest single deviation: row 0
+    assert abs(oracle.marginal_err(T)[0] - (4e-7 + 3e-7)) < 1e-15   # sum |r| + sum |c|
+    # the largest deviation in a column, and a transposed operand would be caught: rows exact, one column pair off
+    T2 = np.full((1, 4, 4), 0.25)
+    T2[0, :, 1] += 2.5e-7
+    T2[0, :, 2] -= 2.5e-7
+    assert abs(oracle.marginal_err_inf(T2)[0] - 1e-6) < 1e-15 and abs(oracle.marginal_err(T2)[0] - 2e-6) < 1e-15
+    T3 = np.transpose(T2, (0, 2, 1)).copy()
+    T3[0, 0, :] += 1e-7                                             # now rows 1, 2 are off by 1e-6 and row 0 by 4e-7, columns by 1e-7
+    assert abs(oracle.marginal_err_inf(T3)[0] - 1e-6) < 1e-15 and abs(oracle.marginal_err(T3)[0] - 2.8e-6) < 1e-15
+    # Err_inf <= Err <= 8 Err_inf (8 marginals) on arbitrary matrices
+    rng = np.random.default_rng(5)
+    X = rng.random((500, 4, 4))
+    e, einf = oracle.marginal_err(X), oracle.marginal_err_inf(X)
+    assert (einf <= e + 1e-15).all() and (e <= 8 * einf + 1e-15).all()

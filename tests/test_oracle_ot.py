@@ -221,3 +221,25 @@ def test_backward_n8_against_80_digit_solve(s):
         assert np.abs(ex - dH[k]).max() < 1e-11
         checked += 1
     assert checked >= 10
+
+
+def test_marginal_err_with_given_marginals_on_a_hand_built_plan():
+    """pin of ot.marginal_err (PAPER.md:323 with marginals a, b): the plan T = a b^T / sum(a) has row sums a and column
+    sums b; moving mass d from entry (0,0) to (0,1) leaves the rows alone and puts columns 0 and 1 off by d each; adding e
+    to entry (2,3) puts row 2 and column 3 off by e each."""
+    a = np.array([[0.5, 1.5, 0.75]])
+    b = np.array([[0.25, 1.0, 0.5, 0.5, 0.5]])                      # both sum to 2.75
+    T = a[:, :, None] * b[:, None, :] / a.sum()
+    assert ot.marginal_err(T, a, b)[0] < 1e-15
+    d, e = 1e-3, 2e-4
+    T[0, 0, 0] -= d
+    T[0, 0, 1] += d
+    assert abs(ot.marginal_err(T, a, b)[0] - 2 * d) < 1e-15
+    T[0, 2, 3] += e
+    assert abs(ot.marginal_err(T, a, b)[0] - (2 * d + 2 * e)) < 1e-15
+    assert abs(ot.marginal_err(T, b=b, a=a)[0] - (2 * d + 2 * e)) < 1e-15
+    # against unit marginals the same plan is off by |a_i - 1| and |b_j - 1| (up to the moved mass): a and b are not ignored
+    T0 = a[:, :, None] * b[:, None, :] / a.sum()
+    n1 = np.ones((1, 3))
+    m1 = np.ones((1, 5))
+    assert abs(ot.marginal_err(T0, n1, m1)[0] - (np.abs(a - 1).sum() + np.abs(b - 1).sum())) < 1e-14
