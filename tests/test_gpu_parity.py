@@ -147,7 +147,22 @@ def test_config5_small(oracle, mode):
 # ---------------------------------------------------------------------------------------------------
 # BASELINE.json's full sizes, in the launch configuration bench.py times: properties over the whole
 # output, the oracle on a sample of matrices
-def _full_size(oracle, H32, G32, P_gpu, n_sample, err_gate, seed):
+def _iteration_counts(H_dev, P_gpu, max_iter, bf16=False):
+    """updates taken by every matrix and the unconverged count, from the diagnostic variant of the same kernel, whose
+    projection must equal the timed variant's bit for bit"""
+    iters = torch.zeros(P_gpu.shape[0], dtype=torch.int32, device="cuda")
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    P2 = (bk.birkhoff4_forward_bf16_ex if bf16 else bk.birkhoff4_forward_ex)(H_dev, max_iter=max_iter, iters=iters,
+                                                                              n_unconverged=unc)
+    assert torch.equal(P2, P_gpu)
+    del P2
+    return host(iters), int(host(unc)[0])
+
+
+def _full_size(oracle, H32, G32, P_gpu, n_sample, err_gate, seed, iters=None):
+    """properties over all B matrices; the oracle on a STRATIFIED sample: n_sample matrices drawn at random plus, when
+    the per-matrix update counts are given, the n_sample / 2 matrices that took the most updates (which include every
+    matrix that ran out of updates or stalled: where a fault that hits one matrix in 10^4 would live)"""
     B = H32.shape[0]
     P = host(P_gpu)
     assert np.isfinite(P).all()
@@ -164,8 +179,13 @@ def _full_size(oracle, H32, G32, P_gpu, n_sample, err_gate, seed):
     # P11: row and column sums of dH vanish (every matrix)
     assert (np.abs(dH.sum(1)).max(1) / scale).max() < 2e-5
     assert (np.abs(dH.sum(2)).max(1) / scale).max() < 2e-5
-    idx = np.sort(np.random.default_rng(seed).choice(B, n_sample, replace=False))
+    idx = np.random.default_rng(seed).choice(B, n_sample, replace=False)
     idx[0], idx[-1] = 0, B - 1
+    if iters is not None:
+        assert iters.shape == (B,)
+        hardest = np.argsort(-iters.astype(np.int64), kind="stable")[:n_sample // 2]
+        idx = np.concatenate([idx, hardest])
+    idx = np.unique(idx)
     P_o, info = oracle.forward(H32[idx].astype(np.float64), return_info=True)
     ok = info["err"] <= oracle.CERTIFY
     assert ok.all(), "oracle uncertified on %d of %d sampled matrices" % ((~ok).sum(), len(ok))
@@ -176,13 +196,16 @@ def _full_size(oracle, H32, G32, P_gpu, n_sample, err_gate, seed):
     assert e1 <= TOL_DH and e2 <= TOL_DH
     err_inf = max(np.abs(P64.sum(2) - 1).max(), np.abs(P64.sum(1) - 1).max())
     assert err_inf <= TOL_ERR
-    return dict(eP=eP, err=err.max(), err_mean=err.mean(), err_inf=err_inf, e1=e1, e2=e2)
+    return dict(eP=eP, err=err.max(), err_mean=err.mean(), err_inf=err_inf, e1=e1, e2=e2, compared=len(idx),
+                most_updates=None if iters is None else int(iters.max()))
 
 
 def test_config2_full_size(oracle):
     c = inputs.make(2)
-    P = bk.birkhoff4_forward(dev(c["H"]))
-    print("config2", _full_size(oracle, c["H"], c["G"], P, 8192, TOL_ERR, 2))
+    Hd = dev(c["H"])
+    P = bk.birkhoff4_forward(Hd)
+    iters, unc = _iteration_counts(Hd, P, 20)
+    print("config2", _full_size(oracle, c["H"], c["G"], P, 8192, TOL_ERR, 2, iters), "unconverged", unc)
 
 
 @pytest.mark.parametrize("s", [10.0, 30.0, 100.0])
@@ -190,8 +213,9 @@ def test_config3_full_size(oracle, s):
     c = inputs.make(3, s=s)
     hist = torch.zeros(64, dtype=torch.int64, device="cuda")
     unc = torch.zeros(1, dtype=torch.int64, device="cuda")
-    P = bk.birkhoff4_forward_ex(dev(c["H"]), max_iter=32, hist=hist, n_unconverged=unc)
-    r = _full_size(oracle, c["H"], c["G"], P, 2048, TOL_ERR, 3)
+    iters = torch.zeros(c["B"], dtype=torch.int32, device="cuda")
+    P = bk.birkhoff4_forward_ex(dev(c["H"]), max_iter=32, iters=iters, hist=hist, n_unconverged=unc)
+    r = _full_size(oracle, c["H"], c["G"], P, 2048, TOL_ERR, 3, host(iters))
     h = host(hist)
     assert h.sum() == c["B"]
     print("config3 s=%g" % s, r, "mean iters %.2f" % ((h * np.arange(64)).sum() / h.sum()), "max", np.nonzero(h)[0].max(),
@@ -202,8 +226,9 @@ def test_config4_full_size(oracle):
     c = inputs.make(4)
     Hb = torch.from_numpy(c["H"].view(np.int16)).cuda().view(torch.bfloat16)
     P = bk.birkhoff4_forward_bf16(Hb)
+    iters, unc = _iteration_counts(Hb, P, 20, bf16=True)
     del Hb
-    print("config4", _full_size(oracle, c["H_f32"], c["G"], P, 4096, TOL_ERR, 4))
+    print("config4", _full_size(oracle, c["H_f32"], c["G"], P, 4096, TOL_ERR, 4, iters), "unconverged", unc)
 
 
 def test_bf16_diagnostics_match_fp32_path():
@@ -222,8 +247,10 @@ def test_bf16_diagnostics_match_fp32_path():
 
 def test_config5_full_size(oracle):
     c = inputs.make(5)
-    P = bk.birkhoff4_forward(dev(c["H"]), max_iter=32)
-    print("config5", _full_size(oracle, c["H"], c["G"], P, 8192, TOL_ERR, 5))
+    Hd = dev(c["H"])
+    P = bk.birkhoff4_forward(Hd, max_iter=32)
+    iters, unc = _iteration_counts(Hd, P, 32)
+    print("config5", _full_size(oracle, c["H"], c["G"], P, 8192, TOL_ERR, 5, iters), "unconverged", unc)
 
 
 # ---------------------------------------------------------------------------------------------------
