@@ -13,10 +13,16 @@
  *
  * Conventions (all entry points)
  *   layout     [B][n][m] row-major contiguous; marginals a [B][n], b [B][m].
- *   sizes      (n, m) in {4, 8} x {4, 8}; anything else returns BIRKHOFF_OT_EINVAL.
+ *   sizes      any 2 <= n, m <= 8; anything else returns BIRKHOFF_OT_EINVAL.  The four sizes {4, 8} x {4, 8} have
+ *              kernels of their own (vector loads, tuned register budgets).  Every other size runs inside the
+ *              next of those tiles: rows beyond n carry mass 0 and columns beyond m carry mass 0 and no entries
+ *              (a zero marginal is outside the domain of eq. (5), so the padding is kept out of
+ *              the formulas by construction rather than passed through them), scalar loads and stores; correct
+ *              to the same gates, not tuned.
  *   pointers   DEVICE pointers owned by the caller; the library neither allocates nor synchronises; every call
  *              is asynchronous on `stream` (a cudaStream_t; 0 = the legacy default stream).
- *   alignment  every matrix pointer must be 32-byte aligned (else BIRKHOFF_OT_EINVAL).
+ *   alignment  every matrix pointer must be 32-byte aligned for the sizes {4, 8} x {4, 8} (256-bit accesses); the
+ *              other sizes are accessed float by float and need 4-byte alignment only (else BIRKHOFF_OT_EINVAL).
  *   aliasing   T == C and D == G are allowed as exact aliases; partial overlap is undefined.
  *   marginals  a and b both NULL: all ones (needs n == m).  Otherwise both given, positive, sum a = sum b
  *              (PAPER.md:91-93); not checked.

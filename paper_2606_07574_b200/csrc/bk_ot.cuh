@@ -71,6 +71,48 @@ BK4_DEV void load_all(const float* p, float (&X)[N * M]) {
     }
 }
 
+// ---- sizes other than {4, 8} x {4, 8} (PAD instances): an n x m problem, 2 <= n <= N, 2 <= m <= M, sits in the N x M
+// register tile.  Rows i >= n are padding with mass a_i = 0; the last real column, m-1, sits in slot M-1 (the ground
+// of the gauge and of the Laplacian must be a real column) and the slots m-1 .. M-2 are padding with b_j = 0 and
+// E_ij = 0: a zero marginal is outside the domain of eq. (5), so such rows and columns are not run
+// through the formulas but carry no mass by construction (T_ij = 0 exactly) and are never stored.
+struct OtShape {
+    int n, m;
+};
+template <int M>
+BK4_DEV bool pad_slot(OtShape sh, int j) { return j >= sh.m - 1 && j < M - 1; }
+template <int M>
+BK4_DEV int slot_column(OtShape sh, int j) { return j == M - 1 ? sh.m - 1 : j; }
+
+// the costs of an n x m problem ([n][m] row-major, scalar loads: rows of odd length are not aligned) into the tile;
+// a padding entry repeats the first entry of its row (of row 0 for a padding row): finite whenever the problem is,
+// inside the problem's range, and never the row's only maximum
+template <int N, int M>
+BK4_DEV void load_padded(const float* p, OtShape sh, float (&X)[N * M]) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const float* row = p + (i < sh.n ? i : 0) * sh.m;
+#pragma unroll
+        for (int j = 0; j < M; ++j) X[i * M + j] = row[pad_slot<M>(sh, j) ? 0 : slot_column<M>(sh, j)];
+    }
+}
+// T or G of the backward: padding entries are zero
+template <int N, int M>
+BK4_DEV void load_padded_zero(const float* p, OtShape sh, float (&X)[N * M]) {
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+#pragma unroll
+        for (int j = 0; j < M; ++j)
+            X[i * M + j] = (i < sh.n && !pad_slot<M>(sh, j)) ? p[i * sh.m + slot_column<M>(sh, j)] : 0.0f;
+}
+template <int M>
+BK4_DEV void store_padded_row(float* p, OtShape sh, int i, const float (&x)[M]) {
+    if (i >= sh.n) return;
+#pragma unroll
+    for (int j = 0; j < M; ++j)
+        if (!pad_slot<M>(sh, j)) p[i * sh.m + slot_column<M>(sh, j)] = x[j];
+}
+
 // index of the edge weight W_jk, j < k < M, in the packed upper triangle
 template <int M>
 BK4_DEV constexpr int tri(int j, int k) {
@@ -145,7 +187,7 @@ BK4_DEV void solve_laplacian(float (&W)[M * (M - 1) / 2], const float (&g)[M], f
 
 // One streamed evaluation at v: column sums c_j = sum_i T_ij, and (HESS) the packed edge weights
 // W_jk = sum_i T_ij T_ik / a_i, with T_ij = a_i E_ij v_j / sum_k E_ik v_k and v_{M-1} = 1.
-template <int N, int M, bool UNIT, bool HESS>
+template <int N, int M, bool UNIT, bool HESS, bool PAD = false>
 BK4_DEV void ot_eval(const float (&E)[N * M], const float (&v)[M - 1], const float (&a)[N], float (&c)[M],
                      float (&W)[M * (M - 1) / 2]) {
 #pragma unroll
@@ -173,7 +215,8 @@ BK4_DEV void ot_eval(const float (&E)[N * M], const float (&v)[M - 1], const flo
             c[j] += x[j];
         }
         if constexpr (HESS) {
-            const float ia = UNIT ? 1.0f : rcp_approx(a[i]);
+            float ia = UNIT ? 1.0f : rcp_approx(a[i]);
+            if constexpr (PAD) ia = a[i] > 0.0f ? ia : 0.0f;  // a padding row: T_i. = 0, and 0 x (1 / 0) must stay 0
 #pragma unroll
             for (int j = 0; j < M - 1; ++j) {
                 const float tj = UNIT ? x[j] : x[j] * ia;
@@ -239,13 +282,22 @@ struct OtStats {
 // The whole forward for one problem.  Cg: this problem's N x M costs (or logits) in global memory, a, b: its
 // marginals in registers (ignored when UNIT), T: where the result goes.  tol_rel: the stop threshold on
 // Err_ab / sum(a) ... as an absolute threshold on the column part of Err_ab (rows are exact by construction).
-template <int N, int M, bool UNIT>
+template <int N, int M, bool UNIT, bool PAD = false>
 BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const float (&a)[N], const float (&b)[M], float tol_abs,
-                               int max_iter, float* Tg) {
+                               int max_iter, float* Tg, OtShape sh = OtShape{N, M}) {
+    static_assert(!(UNIT && PAD), "a padded problem carries its marginals (zeros on the padding)");
     float E[N * M], v[M - 1], vprev[M - 1], bl[M - 1], c[M], W[M * (M - 1) / 2];
+    auto load_costs = [&](float(&X)[N * M]) {
+        if constexpr (PAD) load_padded<N, M>(Cg, sh, X);
+        else load_all<N, M>(Cg, X);
+    };
+    auto store_result_row = [&](int i, const float(&x)[M]) {
+        if constexpr (PAD) store_padded_row<M>(Tg, sh, i, x);
+        else store_row<M>(Tg + i * M, x);
+    };
     // range of the costs decides the continuation schedule
     float lo = kInf, hi = -kInf, suma = 0.0f;
-    load_all<N, M>(Cg, E);
+    load_costs(E);
 #pragma unroll
     for (int i = 0; i < N; ++i) {
 #pragma unroll
@@ -262,7 +314,7 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
 #pragma unroll
         for (int j = 0; j < M; ++j) x[j] = kNaN;
 #pragma unroll
-        for (int i = 0; i < N; ++i) store_row<M>(Tg + i * M, x);
+        for (int i = 0; i < N; ++i) store_result_row(i, x);
         return OtStats{0, false};
     }
     const float lam = kOtLam * suma * (1.0f / N);
@@ -277,8 +329,16 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
     OtStats st = {0, false};
     bool finite = true;
     for (bool first = true;; eta_s *= 0.5f, --stages, first = false) {
-        if (!first) load_all<N, M>(Cg, E);  // a later stage: the costs again (through L2)
+        if (!first) load_costs(E);  // a later stage: the costs again (through L2)
         finite = ot_exponentials<N, M>(sign / eta_s, bl, E) && finite;
+        if constexpr (PAD) {  // a padding column carries no mass
+#pragma unroll
+            for (int j = 0; j < M - 1; ++j)
+                if (pad_slot<M>(sh, j)) {
+#pragma unroll
+                    for (int i = 0; i < N; ++i) E[i * M + j] = 0.0f;
+                }
+        }
 #pragma unroll
         for (int j = 0; j < M - 1; ++j) v[j] = 1.0f;
         // Sinkhorn sweeps in the scaling form of eq. (2) PAPER.md:76 with marginals: u = a / (E v), v = b / (E^T u), gauge
@@ -294,7 +354,7 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
             d[j] = 0.0f;
         }
         for (;;) {
-            ot_eval<N, M, UNIT, true>(E, v, a, c, W);
+            ot_eval<N, M, UNIT, true, PAD>(E, v, a, c, W);
             float g[M], err = 0.0f;
 #pragma unroll
             for (int j = 0; j < M; ++j) {
@@ -314,10 +374,13 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
                     continue;
                 }
                 if (st.iters < max_iter && newton_trial) {
-                    ot_eval<N, M, UNIT, false>(E, vprev, a, c, W);
+                    ot_eval<N, M, UNIT, false, PAD>(E, vprev, a, c, W);
                     const float t = (UNIT ? 1.0f : b[M - 1]) * rcp_approx(c[M - 1]);
 #pragma unroll
-                    for (int j = 0; j < M - 1; ++j) v[j] = vprev[j] * ((UNIT ? 1.0f : b[j]) * rcp_approx(c[j] * t));
+                    for (int j = 0; j < M - 1; ++j) {
+                        v[j] = vprev[j] * ((UNIT ? 1.0f : b[j]) * rcp_approx(c[j] * t));
+                        if constexpr (PAD) v[j] = pad_slot<M>(sh, j) ? vprev[j] : v[j];  // c_j = b_j = 0 there
+                    }
                     newton_trial = 0u, sink_trial = 1u;
                     ++st.iters;
                     continue;
@@ -346,7 +409,10 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
         if (stages <= 0) break;
         // next stage: eta halves, so potentials / eta double: beta/eta <- 2 (beta/eta + log2 v)
 #pragma unroll
-        for (int j = 0; j < M - 1; ++j) bl[j] = 2.0f * (bl[j] + lg2_approx(v[j]));
+        for (int j = 0; j < M - 1; ++j) {
+            bl[j] = 2.0f * (bl[j] + lg2_approx(v[j]));
+            if constexpr (PAD) bl[j] = pad_slot<M>(sh, j) ? 0.0f : bl[j];  // (a sweep leaves v_j = 0 on a padding column)
+        }
     }
     // the result: rows at the final v
 #pragma unroll
@@ -363,7 +429,7 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
         const float ar = UNIT ? r : a[i] * r;
 #pragma unroll
         for (int j = 0; j < M; ++j) x[j] = finite ? x[j] * ar : kNaN;
-        store_row<M>(Tg + i * M, x);
+        store_result_row(i, x);
     }
     st.converged = st.converged && finite;
     return st;
@@ -373,11 +439,16 @@ BK4_DEV OtStats ot_forward_one(const float* Cg, float sign, float eta, const flo
 // Delta w = mu_c - T_{-M}^T (mu_r / a), w_M = 0, Delta = diag(c) - T_{-M}^T diag(a)^{-1} T_{-M} as a grounded Laplacian,
 // D_ij = out_scale T_ij ((mu_r_i - (T w)_i) / a_i + w_j - G_ij),  out_scale = 1/eta for dl/dC, -1 for dl/dH of the
 // Birkhoff projection.  The row marginals a are those of the given T.
-template <int N, int M>
-BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, float* Dg) {
+template <int N, int M, bool PAD = false>
+BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, float* Dg, OtShape sh = OtShape{N, M}) {
     float T[N * M], G[N * M], W[M * (M - 1) / 2], mur[N], ia[N], rhs[M], w[M - 1];
-    load_all<N, M>(Tg, T);
-    load_all<N, M>(Gg, G);  // D may alias G: all of G is in registers before anything is written
+    if constexpr (PAD) {
+        load_padded_zero<N, M>(Tg, sh, T);
+        load_padded_zero<N, M>(Gg, sh, G);
+    } else {
+        load_all<N, M>(Tg, T);
+        load_all<N, M>(Gg, G);  // D may alias G: all of G is in registers before anything is written
+    }
 #pragma unroll
     for (int q = 0; q < M * (M - 1) / 2; ++q) W[q] = 0.0f;
 #pragma unroll
@@ -394,6 +465,7 @@ BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, 
         suma += ai;
         ia[i] = rcp_approx(ai);
         ia[i] = fmaf(ia[i], fmaf(-ai, ia[i], 1.0f), ia[i]);
+        if constexpr (PAD) ia[i] = ai > 0.0f ? ia[i] : 0.0f;  // a padding row: everything it contributes is 0
         mur[i] = mr;
         const float mra = mr * ia[i];
 #pragma unroll
@@ -417,7 +489,8 @@ BK4_DEV void ot_backward_one(const float* Tg, const float* Gg, float out_scale, 
         const float vi = (mur[i] - tw) * ia[i];
 #pragma unroll
         for (int j = 0; j < M; ++j) d[j] = out_scale * T[i * M + j] * ((vi - G[i * M + j]) + (j < M - 1 ? w[j] : 0.0f));
-        store_row<M>(Dg + i * M, d);
+        if constexpr (PAD) store_padded_row<M>(Dg, sh, i, d);
+        else store_row<M>(Dg + i * M, d);
     }
 }
 

@@ -89,7 +89,9 @@ def test_birkhoff8_properties_and_edges():
     assert L.birkhoff8_forward(p, p, -1, 1e-6, 20, None, None, None) == 1
     assert L.birkhoff8_forward(None, p, 4, 1e-6, 20, None, None, None) == 1
     assert L.birkhoff8_forward(ctypes.c_void_p(X.data_ptr() + 4), p, 1, 1e-6, 20, None, None, None) == 1
-    assert L.entropic_ot_forward(p, None, None, p, 4, 5, 5, 1.0, 1e-6, 20, None, None, None) == 1     # unsupported size
+    assert L.entropic_ot_forward(p, None, None, p, 4, 9, 9, 1.0, 1e-6, 20, None, None, None) == 1     # unsupported size (> 8)
+    assert L.entropic_ot_forward(p, p, p, p, 4, 1, 4, 1.0, 1e-6, 20, None, None, None) == 1           # unsupported size (< 2)
+    assert L.entropic_ot_backward(p, p, p, 4, 4, 9, 1.0, None) == 1
     assert L.entropic_ot_forward(p, None, None, p, 4, 4, 8, 1.0, 1e-6, 20, None, None, None) == 1     # unit marginals, n != m
     assert L.entropic_ot_forward(p, p, None, p, 4, 4, 4, 1.0, 1e-6, 20, None, None, None) == 1        # one marginal missing
     assert L.entropic_ot_forward(p, None, None, p, 4, 4, 4, 0.0, 1e-6, 20, None, None, None) == 1     # eta = 0
@@ -177,3 +179,77 @@ def test_ot_inf_cost_gives_nan_for_that_problem_only():
     good = np.ones(300, bool)
     good[[7, 9, 11]] = False
     assert np.isnan(Tn[~good]).all() and np.array_equal(Tn[good], T[good]) and int(unc.item()) == 3
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-3 at every size 2 <= n, m <= 8 (PAPER.md:83-168 is written for any n x m; eq. (13)): sizes other
+# than {4, 8} x {4, 8} run padded inside the next tile, the padding carrying no mass
+RAGGED = [(3, 5), (5, 8), (6, 6), (2, 2), (7, 3), (5, 4), (2, 8), (8, 2), (3, 3), (4, 7), (8, 7)]
+
+
+@pytest.mark.parametrize("n,m", RAGGED)
+@pytest.mark.parametrize("s,eta", [(1.0, 1.0), (3.0, 0.5), (10.0, 1.0)])
+def test_entropic_ot_parity_any_size(n, m, s, eta):
+    B = 1024 + 5
+    Cm, a, b, G = inputs.ot_problem(B, n, m, s, config=9, sub=100 + n * 10 + m)
+    a64, b64 = a.astype(np.float64), b.astype(np.float64)
+    b64 = b64 * (a64.sum(1, keepdims=True) / b64.sum(1, keepdims=True))
+    T_o, info = ot.forward(Cm, a64, b64, eta, return_info=True)
+    assert info["uncertified"] == 0
+    unc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    tol = 2e-6 * max(n, m) / 4
+    # guard cells on both sides of the output: a padded tile must not write outside its n x m problem
+    buf = torch.full((B + 2, n, m), 7.0, device="cuda")
+    Td = bk.entropic_ot_forward(dev(Cm), dev(a), dev(b), buf[1:B + 1], eta=eta, tol=tol, max_iter=80, n_unconverged=unc)
+    assert (host(buf[0]) == 7.0).all() and (host(buf[B + 1]) == 7.0).all()
+    T = host(Td).astype(np.float64)
+    assert np.isfinite(T).all() and T.min() >= 0
+    eT = np.abs(T - T_o).max() / a.max()
+    err = ot.marginal_err(T, a, b)
+    mism = np.abs(a64.sum(1) - b.astype(np.float64).sum(1)).max()
+    print("ot %dx%d s=%g eta=%g: eT %.2e Err max %.2e  unconverged %d" % (n, m, s, eta, eT, err.max(), int(unc.item())))
+    assert eT <= 1e-5
+    assert err.max() <= max(tol, 2e-6) + mism and int(unc.item()) == 0
+    dbuf = torch.full((B + 2, n, m), 7.0, device="cuda")
+    Dd = bk.entropic_ot_backward(Td.contiguous(), dev(G), dbuf[1:B + 1], eta=eta)
+    assert (host(dbuf[0]) == 7.0).all() and (host(dbuf[B + 1]) == 7.0).all()
+    D = host(Dd).astype(np.float64)
+    D_o = ot.backward(T_o, G.astype(np.float64), eta)
+    e1, e2 = d_errors(D * eta, D_o * eta, G)
+    assert np.isfinite(D).all() and e1 <= 1e-4 and e2 <= 1e-4 * a.max(), (e1, e2)
+
+
+@pytest.mark.parametrize("n", [2, 3, 5, 6, 7])
+def test_birkhoff_projection_any_n(n):
+    """unit marginals (a = b = NULL) at sizes other than 4 and 8: the n x n Birkhoff projection of exp(H), C = -H"""
+    H, G = inputs.normal_n(2048 + 1, n, 3.0, config=8, sub=n)
+    P_o = ot.birkhoff_forward(H.astype(np.float64))
+    P = host(bk.entropic_ot_forward(dev(-H), tol=1e-6 * max(n, 4) / 4, max_iter=60)).astype(np.float64)
+    assert np.abs(P - P_o).max() <= 1e-5
+    assert ot.marginal_err(P).max() <= 1e-6 * max(n, 4) / 4 + 1e-7 * n
+    dH = -host(bk.entropic_ot_backward(dev(P.astype(np.float32)), dev(G))).astype(np.float64)
+    dH_o = ot.birkhoff_backward(P_o, G.astype(np.float64))
+    e1, e2 = d_errors(dH, dH_o, G)
+    assert e1 <= 1e-4 and e2 <= 1e-4, (e1, e2)
+
+
+def test_two_by_two_closed_form_gpu():
+    """2 x 2 with general marginals: T = [[t, a1-t], [b1-t, a2-b1+t]] with t (a2-b1+t) = K (a1-t)(b1-t),
+    K = exp(-(C11+C22-C12-C21)/eta): the quadratic solved in fp64 here, not by the oracle"""
+    rng = np.random.default_rng(4)
+    B, eta = 999, 0.8
+    C = (rng.normal(size=(B, 2, 2)) * 3).astype(np.float32)
+    a = rng.uniform(0.2, 2.0, size=(B, 2)).astype(np.float32)
+    b1 = (rng.uniform(0.05, 0.95, size=B) * a.astype(np.float64).sum(1))
+    b = np.stack([b1, a.astype(np.float64).sum(1) - b1], 1).astype(np.float32)
+    T = host(bk.entropic_ot_forward(dev(C), dev(a), dev(b), eta=eta, tol=1e-6, max_iter=60)).astype(np.float64)
+    C64, a64, b64 = C.astype(np.float64), a.astype(np.float64), b.astype(np.float64)
+    K = np.exp(-(C64[:, 0, 0] + C64[:, 1, 1] - C64[:, 0, 1] - C64[:, 1, 0]) / eta)
+    a1, a2, bb = a64[:, 0], a64[:, 1], b64[:, 0]
+    A, Bq, Cq = 1 - K, (a2 - bb) + K * (a1 + bb), -K * a1 * bb
+    disc = np.sqrt(Bq * Bq - 4 * A * Cq)
+    t = np.where(np.abs(A) < 1e-12, -Cq / Bq, (-Bq + disc) / (2 * A))
+    t2 = np.where(np.abs(A) < 1e-12, t, (-Bq - disc) / (2 * A))
+    lo, hi = np.maximum(0, bb - a2), np.minimum(a1, bb)
+    t = np.where((t >= lo - 1e-12) & (t <= hi + 1e-12), t, t2)
+    assert np.abs(T[:, 0, 0] - t).max() <= 1e-5 and np.abs(T.sum(2) - a64).max() <= 2e-6
