@@ -141,6 +141,22 @@ int birkhoff4_forward_mix_bf16(const float* H, const uint16_t* X, uint16_t* Y, f
                                int max_iter, birkhoff4_stream_t stream);
 
 /*
+ * Backward of the fused consumer: everything the training step needs from the mix Y_b = P_b X_b in one
+ * kernel, with P_b = proj^KL_{B_4}(exp(H_b)) projected again from the logits (recompute-style), so
+ * that neither P nor dL/dP ever goes through HBM:
+ *     dX_b = P_b^T dY_b,     G_b = dY_b X_b^T  (= dL/dP_b, a 4 x 4 matrix of C-long dot products, fp32 accumulation),
+ *     dH_b = dL/dH_b from (P_b, G_b) by the formula of birkhoff4_backward.
+ * H: device fp32 [B][4][4]; X, dY, dX: device [B][4][C] row-major, fp32 or bf16 bit patterns (round-to-nearest-even on
+ * store), 16-byte aligned, C a multiple of 4 (fp32) or 8 (bf16); dX must not alias X or dY; dH: device fp32 [B][4][4]
+ * (dH == H is allowed); P: device fp32 [B][4][4] or NULL, written only if given.  tol, max_iter as in birkhoff4_forward:
+ * with the same values P equals birkhoff4_forward's bit for bit.  Errors as for birkhoff4_forward_mix.
+ */
+int birkhoff4_backward_mix(const float* H, const float* X, const float* dY, float* dX, float* dH, float* P, int64_t B, int C,
+                           float tol, int max_iter, birkhoff4_stream_t stream);
+int birkhoff4_backward_mix_bf16(const float* H, const uint16_t* X, const uint16_t* dY, uint16_t* dX, float* dH, float* P,
+                                int64_t B, int C, float tol, int max_iter, birkhoff4_stream_t stream);
+
+/*
  * Sinkhorn-Knopp baseline (eq. (2)): K = exp(H) (row-max shifted, which the first row
  * normalisation cancels), then n_iter x (rows /= row sums; columns /= column sums).  n_iter = 20 is the
  * "Sinkhorn-20" of PAPER.md:32, 319.  Reported baseline only.

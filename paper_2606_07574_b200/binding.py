@@ -44,6 +44,8 @@ def lib():
             "forward_backward": [vp, vp, vp, vp, i64, f32, ci, vp],
             "forward_mix": [vp, vp, vp, vp, i64, ci, f32, ci, vp],
             "forward_mix_bf16": [vp, vp, vp, vp, i64, ci, f32, ci, vp],
+            "backward_mix": [vp, vp, vp, vp, vp, vp, i64, ci, f32, ci, vp],
+            "backward_mix_bf16": [vp, vp, vp, vp, vp, vp, i64, ci, f32, ci, vp],
             "sinkhorn": [vp, vp, i64, ci, vp],
             "forward_host": [vp, vp, i64, f32, ci],
             "backward_host": [vp, vp, vp, i64],
@@ -212,6 +214,28 @@ def birkhoff4_forward_mix(H, X, Y=None, P=None, tol=1e-6, max_iter=20, want_P=Fa
     with torch.cuda.device(H.device):
         _check(fn(_ptr(H), _ptr(X), _ptr(Y), _ptr(P), B, C, tol, max_iter, _stream(stream, H.device)))
     return Y, P
+
+
+def birkhoff4_backward_mix(H, X, dY, dX=None, dH=None, P=None, tol=1e-6, max_iter=20, want_P=False, stream=None):
+    """backward of the fused consumer in one kernel: dX[b] = P[b]^T dY[b] and dH[b] = dL/dH[b] from G[b] = dY[b] X[b]^T, with
+    P[b] = proj(exp(H[b])) projected again from the logits; X, dY [B,4,C] fp32 or bfloat16 CUDA.  Returns (dX, dH, P or None)"""
+    H = _dev(H, torch.float32, "H")
+    B = _batch(H, 16, "H")
+    if not isinstance(X, torch.Tensor) or X.dtype not in (torch.float32, torch.bfloat16):
+        raise Birkhoff4Error("X must be a float32 or bfloat16 tensor")
+    X = _dev(X, X.dtype, "X", like=H)
+    if X.dim() != 3 or X.shape[0] != B or X.shape[1] != 4:
+        raise Birkhoff4Error("X must be [B,4,C]")
+    C = X.shape[2]
+    dY = _dev(dY, X.dtype, "dY", X.numel(), H)
+    dX = _out(dX, X, "dX", X.dtype)
+    dH = _out(dH, H, "dH")
+    if want_P or P is not None:
+        P = _out(P, H, "P")
+    fn = lib().birkhoff4_backward_mix if X.dtype == torch.float32 else lib().birkhoff4_backward_mix_bf16
+    with torch.cuda.device(H.device):
+        _check(fn(_ptr(H), _ptr(X), _ptr(dY), _ptr(dX), _ptr(dH), _ptr(P), B, C, tol, max_iter, _stream(stream, H.device)))
+    return dX, dH, P
 
 
 def birkhoff4_sinkhorn(H, P=None, n_iter=20, stream=None):

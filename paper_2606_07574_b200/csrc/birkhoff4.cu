@@ -135,6 +135,58 @@ __global__ void __launch_bounds__(kThreads, 512 / kThreads) forward_mix_kernel(
         mix_tokens<XBF16>(s_col, t, ntok - t, X + (size_t)(tok0 + t) * 4 * C, Y + (size_t)(tok0 + t) * 4 * C, C);
 }
 
+// ---------------------------------------------------------------- backward of the fused consumer
+// One block = kMixTokens tokens, as in forward_mix_kernel.  Phase 1: thread t projects token t's logits again
+// (recompute-style: the backward needs nothing of the forward but its result) and leaves P_t in its
+// shared-memory column.  Phase 2: each of the block's warps takes every fourth token and streams its x and dy once:
+// dx = P^T dy goes out as it is formed, G = dy x^T = dL/dP is summed over the warp and left in shared memory.
+// Phase 3: thread t turns (P_t, G_t) into dL/dH_t by the implicit-function-theorem formula, the same
+// backward_ift as birkhoff4_backward.  Neither P nor G ever goes through HBM.
+template <bool XBF16>
+__global__ void __launch_bounds__(kThreads, 512 / kThreads) backward_mix_kernel(
+    const float* __restrict__ H, const typename MixVec<XBF16>::elem* __restrict__ X, const typename MixVec<XBF16>::elem* __restrict__ dY,
+    typename MixVec<XBF16>::elem* __restrict__ dX, float* __restrict__ dH, float* __restrict__ P, int64_t B, int C, float tol_i,
+    int max_iter, float lp_range) {
+    pdl_wait_and_trigger();
+    __shared__ float s_col[16 * kThreads];
+    __shared__ float s_G[16 * kThreads];
+    float* const sm = s_col + threadIdx.x;
+    const int64_t tok0 = (int64_t)blockIdx.x * kMixTokens;
+    const int64_t b = tok0 + threadIdx.x;
+    const bool valid = b < B;
+    const int64_t idx = valid ? b : B - 1;
+    auto load = [&](float(&h)[16]) { load_matrix(H + 16 * idx, h); };
+    auto commit = [&](const float(&out)[16]) {
+        if (P) store_matrix(P + 16 * idx, out);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) sm[q * kSmStride] = out[q];
+    };
+    auto record = [](int, bool) {};
+    project_one<false>(load, valid, sm, tol_i, max_iter, lp_range, commit, record);
+    __syncthreads();
+    const int ntok = (int)((B - tok0 < kMixTokens) ? B - tok0 : kMixTokens);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int t = warp; t < ntok; t += kThreads / 32) {
+        float G[16];
+        const size_t off = (size_t)(tok0 + t) * 4 * C;
+        mix_backward_token<XBF16>(s_col, t, X + off, dY + off, dX + off, C, G);
+#pragma unroll
+        for (int q = 0; q < 16; ++q)
+            if (lane == q) s_G[q * kSmStride + t] = G[q];
+    }
+    __syncthreads();
+    if (valid) {
+        float p[16], g[16], d[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            p[q] = sm[q * kSmStride];
+            g[q] = s_G[q * kSmStride + threadIdx.x];
+        }
+        backward_ift(p, g, d);
+        store_matrix(dH + 16 * idx, d);
+    }
+}
+
 // ---------------------------------------------------------------- backward kernel (HBM-bound: 192 B per matrix)
 __global__ void __launch_bounds__(kThreadsBwd) backward_kernel(const float* __restrict__ P, const float* __restrict__ dP,
                                                             float* __restrict__ dH, int64_t B) {
@@ -365,6 +417,19 @@ static int run_host_static(const float* H_host, float* P_host, int64_t B, float 
     return rc;
 }
 
+template <bool XBF16>
+static int launch_mix_backward(const float* H, const void* X, const void* dY, void* dX, float* dH, float* P, int64_t B, int C,
+                               float tol, int max_iter, cudaStream_t stream) {
+    using E = typename MixVec<XBF16>::elem;
+    if (B < 0 || !(tol >= 0.0f) || max_iter < 0 || C < 1 || C % MixVec<XBF16>::kElems) return BIRKHOFF4_EINVAL;
+    if (B == 0) return BIRKHOFF4_OK;
+    if (!H || !X || !dY || !dX || !dH || misaligned(H) || misaligned(dH) || misaligned(P) || (reinterpret_cast<uintptr_t>(X) & 15u) ||
+        (reinterpret_cast<uintptr_t>(dY) & 15u) || (reinterpret_cast<uintptr_t>(dX) & 15u))
+        return BIRKHOFF4_EINVAL;
+    return cuda_rc(launch(backward_mix_kernel<XBF16>, grid_for(B, kMixTokens), kThreads, stream, H, (const E*)X, (const E*)dY, (E*)dX,
+                          dH, P, B, C, internal_tol(tol), max_iter, kLpRange));
+}
+
 }  // namespace bk4
 
 // =================================================================== C ABI
@@ -410,6 +475,16 @@ int birkhoff4_forward_mix(const float* H, const float* X, float* Y, float* P, in
 int birkhoff4_forward_mix_bf16(const float* H, const uint16_t* X, uint16_t* Y, float* P, int64_t B, int C, float tol,
                                int max_iter, birkhoff4_stream_t stream) {
     return launch_mix<true>(H, X, Y, P, B, C, tol, max_iter, (cudaStream_t)stream);
+}
+
+int birkhoff4_backward_mix(const float* H, const float* X, const float* dY, float* dX, float* dH, float* P, int64_t B, int C,
+                           float tol, int max_iter, birkhoff4_stream_t stream) {
+    return launch_mix_backward<false>(H, X, dY, dX, dH, P, B, C, tol, max_iter, (cudaStream_t)stream);
+}
+
+int birkhoff4_backward_mix_bf16(const float* H, const uint16_t* X, const uint16_t* dY, uint16_t* dX, float* dH, float* P,
+                                int64_t B, int C, float tol, int max_iter, birkhoff4_stream_t stream) {
+    return launch_mix_backward<true>(H, X, dY, dX, dH, P, B, C, tol, max_iter, (cudaStream_t)stream);
 }
 
 int birkhoff4_backward(const float* P, const float* dP, float* dH, int64_t B, birkhoff4_stream_t stream) {

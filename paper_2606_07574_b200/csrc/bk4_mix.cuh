@@ -105,4 +105,56 @@ BK4_DEV void mix_tokens(const float* sP, int t0, int n, const typename MixVec<XB
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Backward of the mix for ONE token, by one warp (birkhoff4_backward_mix): with y_i = sum_j P_ij x_j,
+//     dx_j = sum_i P_ij dy_i          (written as it is formed),
+//     G_ij = dL/dP_ij = sum_c dy_i[c] x_j[c]   (returned, summed over the warp: every lane holds all 16 sums).
+// Lane l takes the 16-byte slices l, l + 32, ... of each of the eight streams (4 of x, 4 of dy).  sP: as in mix_tokens.
+template <bool XBF16>
+BK4_DEV void mix_backward_token(const float* sP, int t, const typename MixVec<XBF16>::elem* __restrict__ x,
+                                const typename MixVec<XBF16>::elem* __restrict__ dy, typename MixVec<XBF16>::elem* __restrict__ dx,
+                                int C, float (&G)[16]) {
+    using MV = MixVec<XBF16>;
+    constexpr int V = MV::kElems;
+    const int lane = threadIdx.x & 31;
+    float p[16];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        p[q] = sP[q * kSmStride + t];
+        G[q] = 0.0f;
+    }
+    for (int c = lane * V; c < C; c += 32 * V) {
+        typename MV::raw rx[4], rg[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) rx[j] = MV::load_raw(x + (size_t)j * C + c);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) rg[i] = MV::load_raw(dy + (size_t)i * C + c);
+        float xin[4][V], gin[4][V];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            MV::widen(rx[j], xin[j]);
+            MV::widen(rg[j], gin[j]);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int e = 0; e < V; ++e) G[4 * i + j] = fmaf(gin[i][e], xin[j][e], G[4 * i + j]);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            float out[V];
+#pragma unroll
+            for (int e = 0; e < V; ++e)
+                out[e] = fmaf(p[12 + j], gin[3][e], fmaf(p[8 + j], gin[2][e], fmaf(p[4 + j], gin[1][e], p[j] * gin[0][e])));
+            MV::store(dx + (size_t)j * C + c, out);
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) G[q] += __shfl_xor_sync(0xffffffffu, G[q], off);
+    }
+}
+
 }  // namespace bk4

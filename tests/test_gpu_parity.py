@@ -716,6 +716,75 @@ def test_fused_mix_matches_oracle(oracle, B, C, dtype):
     assert none is None and torch.equal(Y2, Y)
 
 
+# backward of the fused consumer (PAPER.md:46-50 differentiated, then section 4.2) in one kernel.  The
+# oracle is the definition: dX = P_o^T dY and G = dY X^T as fp64 matrix products (numpy), dH = the oracle's backward at
+# (P_o, G).
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("B,C", [(1, 8), (129, 64), (1000, 1024), (4097, 200), (300, 4096)])
+def test_fused_mix_backward_matches_oracle(oracle, B, C, dtype):
+    H = inputs.normal(B, 3.0, config=98, sub=B)[0]
+    rng = np.random.Generator(np.random.Philox(key=inputs.SEED + 199 + B))
+    X = rng.standard_normal((B, 4, C), dtype=np.float32)
+    dY = rng.standard_normal((B, 4, C), dtype=np.float32)
+    Hd = dev(H)
+    if dtype == "bf16":
+        Xb, dYb = inputs.f32_to_bf16_bits(X), inputs.f32_to_bf16_bits(dY)
+        X, dY = inputs.bf16_bits_to_f32(Xb), inputs.bf16_bits_to_f32(dYb)          # the oracle sees what the kernel sees
+        Xd = torch.from_numpy(Xb.view(np.int16)).cuda().view(torch.bfloat16)
+        dYd = torch.from_numpy(dYb.view(np.int16)).cuda().view(torch.bfloat16)
+    else:
+        Xd, dYd = dev(X), dev(dY)
+    xbuf = torch.full((B + 2, 4, C), 7.0, device="cuda", dtype=Xd.dtype)
+    hbuf = torch.full((B + 2, 4, 4), 7.0, device="cuda")
+    dX, dH, P = bk.birkhoff4_backward_mix(Hd, Xd, dYd, xbuf[1:B + 1], hbuf[1:B + 1], want_P=True, max_iter=32)
+    for buf in (xbuf, hbuf):                                                       # guard cells
+        assert (buf[0].float() == 7.0).all() and (buf[B + 1].float() == 7.0).all()
+    assert torch.equal(P, bk.birkhoff4_forward(Hd, max_iter=32))                   # the same projection, bit for bit
+    P_o = oracle.forward(H.astype(np.float64))
+    dX_o = np.einsum("bij,bic->bjc", P_o, dY.astype(np.float64))
+    G_o = np.einsum("bic,bjc->bij", dY.astype(np.float64), X.astype(np.float64))
+    dH_o = oracle.backward(P_o, G_o)
+    dXh = host(dX.float()).astype(np.float64)
+    tol = 2.0 ** -8 if dtype == "bf16" else 2e-6
+    assert (np.abs(dXh - dX_o) <= tol * np.maximum(np.abs(dX_o), 1.0) + 1e-6).all()
+    dHh = host(dH).astype(np.float64)
+    assert np.isfinite(dHh).all()
+    e1, e2 = dh_errors(dHh, dH_o, G_o)
+    if B < 256:
+        e1 = 0.0
+    assert e1 <= TOL_DH and e2 <= TOL_DH, (e1, e2)
+    # against the library's own separate calls: G formed by torch in fp32, then birkhoff4_backward
+    G32 = torch.einsum("bic,bjc->bij", dYd.float(), Xd.float()).contiguous()
+    dH_sep = host(bk.birkhoff4_backward(P, G32)).astype(np.float64)
+    assert np.abs(dHh - dH_sep).max() <= 1e-4 * max(np.abs(dH_o).max(), 1.0)
+    dX2, dH2, none = bk.birkhoff4_backward_mix(Hd, Xd, dYd, max_iter=32)             # P not requested: never written
+    assert none is None and torch.equal(dX2, dX) and torch.equal(dH2, dH)
+
+
+def test_fused_mix_backward_edges():
+    H = dev(inputs.normal(64, 1.0, config=98)[0])
+    X = torch.ones((64, 4, 16), device="cuda")
+    L = bk.lib()
+    import ctypes
+    ph, px, pd = ctypes.c_void_p(H.data_ptr()), ctypes.c_void_p(X.data_ptr()), ctypes.c_void_p(torch.empty_like(H).data_ptr())
+    assert L.birkhoff4_backward_mix(ph, px, px, px, pd, None, 64, 6, 1e-6, 20, None) == 1       # C not a multiple of 4
+    assert L.birkhoff4_backward_mix(ph, px, None, px, pd, None, 64, 16, 1e-6, 20, None) == 1    # null dY
+    assert L.birkhoff4_backward_mix(ph, px, px, px, None, None, 64, 16, 1e-6, 20, None) == 1    # null dH
+    assert L.birkhoff4_backward_mix(None, None, None, None, None, None, 0, 16, 1e-6, 20, None) == 0
+    with pytest.raises(bk.Birkhoff4Error):
+        bk.birkhoff4_backward_mix(H, X, torch.ones((63, 4, 16), device="cuda"))
+    Hn = H.clone()
+    Hn[3, 1, 1] = float("nan")
+    dX, dH, _ = bk.birkhoff4_backward_mix(Hn, X, X)
+    assert torch.isnan(dX[3]).all() and torch.isnan(dH[3]).all()
+    ok = torch.ones(64, dtype=torch.bool, device="cuda")
+    ok[3] = False
+    dX0, dH0, _ = bk.birkhoff4_backward_mix(H, X, X)
+    assert torch.equal(dX[ok], dX0[ok]) and torch.equal(dH[ok], dH0[ok])              # the other tokens are untouched
+    e = torch.empty((0, 4, 4), device="cuda")
+    assert bk.birkhoff4_backward_mix(e, torch.empty((0, 4, 16), device="cuda"), torch.empty((0, 4, 16), device="cuda"))[1].shape == (0, 4, 4)
+
+
 def test_fused_mix_edges():
     H = dev(inputs.normal(64, 1.0, config=98)[0])
     X = torch.zeros((64, 4, 16), device="cuda")
