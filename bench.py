@@ -479,6 +479,14 @@ def measure_widenings(torch, bk, inputs, K, R, peak):
     out["fused_mix_bf16"] = {"desc": "B=2^16 tokens, 4 streams x C=1024 bf16: Y = proj(exp(H)) X in one kernel", "us": us,
                              "bytes_per_token": byts, "achieved_GBs": Bm * byts / (us["median"] * 1e-6) / 1e9,
                              "frac": Bm * byts / (us["median"] * 1e-6) / 1e9 / peak, "tokens_per_s": Bm / (us["median"] * 1e-6)}
+    dYs = [torch.randn((Bm, 4, C), device="cuda", generator=g).bfloat16() for _ in range(2)]
+    dHm = torch.empty_like(Hm)
+    us = timer(lambda i: bk.birkhoff4_backward_mix(Hm, Xs[i % 2], dYs[i % 2], Ys[i % 2], dHm, None, TOL, 20))
+    byts = 128 + 3 * 4 * C * 2
+    out["fused_mix_backward_bf16"] = {
+        "desc": "B=2^16 tokens, C=1024 bf16: dX = P^T dY, G = dY X^T, dH from (P, G), P projected again, one kernel", "us": us,
+        "bytes_per_token": byts, "achieved_GBs": Bm * byts / (us["median"] * 1e-6) / 1e9,
+        "frac": Bm * byts / (us["median"] * 1e-6) / 1e9 / peak, "tokens_per_s": Bm / (us["median"] * 1e-6)}
     return out
 
 

@@ -170,9 +170,8 @@ __global__ void __launch_bounds__(kThreads, 512 / kThreads) backward_mix_kernel(
         float G[16];
         const size_t off = (size_t)(tok0 + t) * 4 * C;
         mix_backward_token<XBF16>(s_col, t, X + off, dY + off, dX + off, C, G);
-#pragma unroll
-        for (int q = 0; q < 16; ++q)
-            if (lane == q) s_G[q * kSmStride + t] = G[q];
+        const float total = mix_reduce16(G);
+        if (!(lane & 1)) s_G[mix_entry_of_lane(lane) * kSmStride + t] = total;
     }
     __syncthreads();
     if (valid) {

@@ -108,7 +108,7 @@ BK4_DEV void mix_tokens(const float* sP, int t0, int n, const typename MixVec<XB
 // ---------------------------------------------------------------------------------------------------------------
 // Backward of the mix for ONE token, by one warp (birkhoff4_backward_mix): with y_i = sum_j P_ij x_j,
 //     dx_j = sum_i P_ij dy_i          (written as it is formed),
-//     G_ij = dL/dP_ij = sum_c dy_i[c] x_j[c]   (returned, summed over the warp: every lane holds all 16 sums).
+//     G_ij = dL/dP_ij = sum_c dy_i[c] x_j[c]   (returned as this lane's partial sums: mix_reduce16 adds them over the warp).
 // Lane l takes the 16-byte slices l, l + 32, ... of each of the eight streams (4 of x, 4 of dy).  sP: as in mix_tokens.
 template <bool XBF16>
 BK4_DEV void mix_backward_token(const float* sP, int t, const typename MixVec<XBF16>::elem* __restrict__ x,
@@ -150,11 +150,26 @@ BK4_DEV void mix_backward_token(const float* sP, int t, const typename MixVec<XB
             MV::store(dx + (size_t)j * C + c, out);
         }
     }
+}
+
+// Sum of the 16 partial sums G[.] over the 32 lanes of the warp by a transposing butterfly: at each of the steps
+// xor 16, 8, 4, 2 a lane keeps one half of its values and hands the other half to its partner (8 + 4 + 2 + 1 shuffles),
+// a last step xor 1 completes the sum: 16 shuffles instead of the 80 of sixteen plain butterflies.  Afterwards lane l
+// holds the total of entry mix_entry_of_lane(l) (lanes l and l ^ 1 hold the same one).
+BK4_DEV int mix_entry_of_lane(int lane) { return lane >> 1; }
+BK4_DEV float mix_reduce16(const float (&G)[16]) {
+    const int lane = threadIdx.x & 31;
+    const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4, h2 = lane & 2;
+    float a[8], b[4], c[2];
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
+    for (int k = 0; k < 8; ++k) a[k] = (h16 ? G[k + 8] : G[k]) + __shfl_xor_sync(0xffffffffu, h16 ? G[k] : G[k + 8], 16);
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) G[q] += __shfl_xor_sync(0xffffffffu, G[q], off);
-    }
+    for (int k = 0; k < 4; ++k) b[k] = (h8 ? a[k + 4] : a[k]) + __shfl_xor_sync(0xffffffffu, h8 ? a[k] : a[k + 4], 8);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) c[k] = (h4 ? b[k + 2] : b[k]) + __shfl_xor_sync(0xffffffffu, h4 ? b[k] : b[k + 2], 4);
+    float d = (h2 ? c[1] : c[0]) + __shfl_xor_sync(0xffffffffu, h2 ? c[0] : c[1], 2);
+    d += __shfl_xor_sync(0xffffffffu, d, 1);
+    return d;  // entry 8 [lane & 16] + 4 [lane & 8] + 2 [lane & 4] + [lane & 2] = lane >> 1
 }
 
 }  // namespace bk4
