@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(kThreads, 512 / kThreads) backward_mix_kernel(
     int max_iter, float lp_range) {
     pdl_wait_and_trigger();
     __shared__ float s_col[16 * kThreads];
-    __shared__ float s_G[16 * kThreads];
+    __shared__ float s_G[17 * kThreads];  // token t's entry q at [17 t + q]: conflict-free for the warp that writes it and for phase 3
     float* const sm = s_col + threadIdx.x;
     const int64_t tok0 = (int64_t)blockIdx.x * kMixTokens;
     const int64_t b = tok0 + threadIdx.x;
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(kThreads, 512 / kThreads) backward_mix_kernel(
         const size_t off = (size_t)(tok0 + t) * 4 * C;
         mix_backward_token<XBF16>(s_col, t, X + off, dY + off, dX + off, C, G);
         const float total = mix_reduce16(G);
-        if (!(lane & 1)) s_G[mix_entry_of_lane(lane) * kSmStride + t] = total;
+        if (!(lane & 1)) s_G[17 * t + mix_entry_of_lane(lane)] = total;
     }
     __syncthreads();
     if (valid) {
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(kThreads, 512 / kThreads) backward_mix_kernel(
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             p[q] = sm[q * kSmStride];
-            g[q] = s_G[q * kSmStride + threadIdx.x];
+            g[q] = s_G[17 * threadIdx.x + q];
         }
         backward_ift(p, g, d);
         store_matrix(dH + 16 * idx, d);
