@@ -181,6 +181,8 @@ def contract_line(full):
     line["config"] = {k: c[k] for k in ("workload", "desc", "B_per_gpu", "tol", "max_iter", "l2") if k in c}
     line["roofline"] = {k: rf.get(k) for k in ("kernel", "bound", "achieved", "peak", "unit", "frac", "avg_us", "isolated_us",
                                                "frac_isolated", "bytes_per_launch", "traffic", "peak_source")}
+    wr = rf.get("work_roofline") or {}
+    line["roofline"]["work_bound"], line["roofline"]["work_frac"] = wr.get("bound"), wr.get("frac")   # slower of HBM / FP32 / SFU work
     line["roofline_step"] = {k: full["roofline_step"].get(k) for k in ("bound", "achieved", "peak", "unit", "frac")}
     line["fwd_us"], line["bwd_us"] = full["fwd"]["us"]["median"], full["bwd"]["us"]["median"]
     line["bwd_frac"] = full["roofline_kernels"]["backward_kernel"]["frac"]
@@ -193,9 +195,10 @@ def contract_line(full):
     line["clocks"] = full.get("clocks")
     line["gpu_launches"] = full.get("gpu_launches")
     if full.get("workloads"):
-        # name: [step_us, forward frac of HBM peak, backward frac, max marginal error]
+        # name: [step_us, forward frac of HBM peak, backward frac, max marginal error, forward frac of the work roofline]
         line["per_config"] = {n: [w["step_us"]["median"], w["roofline_kernels"]["forward_kernel"]["frac"],
-                                  w["roofline_kernels"]["backward_kernel"]["frac"], w["max_marginal_err"]]
+                                  w["roofline_kernels"]["backward_kernel"]["frac"], w["max_marginal_err"],
+                                  (w["roofline_kernels"]["forward_kernel"].get("work_roofline") or {}).get("frac")]
                               for n, w in full["workloads"].items() if "@" not in n}
     if full.get("detail_file"):
         line["detail_file"] = full["detail_file"]
@@ -279,6 +282,19 @@ def _rooflines(B, bf16, f_us, b_us, s_us, peak, peak_src, workload, mean_updates
     ach = B * (fb + BWD_BYTES) / (s_us["median"] * 1e-6) / 1e9
     step = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "bytes_per_step": B * (fb + BWD_BYTES),
             "peak_source": peak_src}
+    # north_star's roofline: the slower of the bytes at HBM peak and the executed exp / FMA work at SFU / FP32 peak
+    # (128 FP32 lanes and 16 SFU lanes per clock per SM: B200_PROFILING.md), counts per 32 matrices from the ncu SASS
+    # opcode tables (profiles/traffic.csv).  Unlike issue_diagnostic below it does not count selects, min/max, votes,
+    # shared-memory moves: what separates the kernel from this floor is exactly that overhead plus imperfect overlap.
+    work = ncu_work("forward_kernel", workload)
+    if work:
+        clk = n_sm * sm_mhz * 1e6
+        t = {"hbm": B * fb / (peak * 1e9) * 1e6, "fp32": work[0] * B / (128.0 * clk) * 1e6, "sfu": work[1] * B / (16.0 * clk) * 1e6}
+        bound = max(t, key=t.get)
+        k["forward_kernel"]["work_roofline"] = {
+            "bound": bound, "floor_us": t[bound], "frac": t[bound] / f_us["median"], "hbm_us": t["hbm"], "fp32_us": t["fp32"],
+            "sfu_us": t["sfu"], "fp32_warp_instr_per_32": work[0], "mufu_warp_instr_per_32": work[1],
+            "peak_source": "nominal: 128 FP32 and 16 SFU lanes per clock per SM x %d SMs x %d MHz; HBM: %s" % (n_sm, sm_mhz, peak_src)}
     winst = ncu_warp_inst("forward_kernel", workload)
     if winst:
         issue_peak = 4.0 * n_sm * sm_mhz * 1e6                                 # warp instructions / s
@@ -289,6 +305,19 @@ def _rooflines(B, bf16, f_us, b_us, s_us, peak, peak_src, workload, mean_updates
             "peak_source": "nominal: 4 issue slots per clock per SM x %d SMs x %d MHz (half-rate instructions hold a slot for "
                            "two clocks, profiles/r2_pipe_microbench.md: the attainable fraction is below 1)" % (n_sm, sm_mhz)}
     return k, step
+
+
+def ncu_work(kernel, workload):
+    """(FP32, MUFU) warp instructions per 32 matrices of `kernel` on `workload` from profiles/traffic.csv, or None"""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            k = [x.strip() for x in line.split(",")]
+            if len(k) >= 7 and k[0] == kernel and k[1] == workload:
+                return float(k[5]), float(k[6])
+    return None
 
 
 def ncu_warp_inst(kernel, workload):

@@ -179,7 +179,8 @@ def _canned_bench_result():
     kern = lambda frac: {"bound": "hbm", "achieved": 4673.123456, "peak": 6556.8, "unit": "GB/s", "frac": frac,   # noqa: E731
                          "frac_min_time": 0.72, "frac_of_nominal_7700": 0.61, "avg_us": 28.123456789, "min_us": 27.9,
                          "bytes_per_launch": 134217728, "traffic": 91435776.0, "isolated_us": 31.4, "frac_isolated": 0.652,
-                         "issue_diagnostic": {"bound": "alu", "frac": 0.5, "peak_source": "x" * 300}}
+                         "issue_diagnostic": {"bound": "alu", "frac": 0.5, "peak_source": "x" * 300},
+                         "work_roofline": {"bound": "fp32", "frac": 0.74, "floor_us": 20.6, "peak_source": "y" * 200}}
     wl = {"desc": "B=2^20 fp32, H iid N(0,10^2)", "step_us": us, "forward_us": us, "backward_us": us, "max_marginal_err": 9.6e-7,
           "roofline_kernels": {"forward_kernel": kern(0.48), "backward_kernel": kern(1.01)},
           "update_histogram": {str(k): 0.01 for k in range(40)}}
@@ -231,4 +232,5 @@ def test_bench_contract_line_is_compact_and_complete():
     assert {"value", "unit", "cores", "kind", "sample"} == set(line["cpu_baseline"])
     assert {"value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step"} <= set(line["e2e"])
     assert sorted(line["per_config"]) == ["config3_s10", "config3_s100", "config3_s30", "config4", "config5"]
-    assert len(line["per_config"]["config5"]) == 4
+    assert len(line["per_config"]["config5"]) == 5
+    assert line["roofline"]["work_bound"] == "fp32" and abs(line["roofline"]["work_frac"] - 0.74) < 1e-3
